@@ -1,0 +1,435 @@
+"""Pins of the CPU oracle against things other than itself (paper identities, closed forms,
+quadrature, brute force, published RNG vectors).  CPU only (-m "not gpu").
+
+Each test names the passage of PAPER.md (or the DESIGN.md reading) it checks.
+"""
+import math
+import os
+
+import numpy as np
+import pytest
+from scipy import integrate
+
+import oracle
+from paper_1609_07936_b200 import workloads as wl
+
+GOLDEN = os.path.join(os.path.dirname(__file__), "golden")
+TWO_PI = 2.0 * math.pi
+
+
+# ----------------------------------------------------------------------------- Philox (G14)
+def _py_philox(ctr, key):
+    """Independent restatement of Philox4x32-10 (python integers)."""
+    c, k = list(ctr), list(key)
+    for _ in range(10):
+        p0, p1 = 0xD2511F53 * c[0], 0xCD9E8D57 * c[2]
+        c = [(p1 >> 32) ^ c[1] ^ k[0], p1 & 0xFFFFFFFF, (p0 >> 32) ^ c[3] ^ k[1], p0 & 0xFFFFFFFF]
+        k = [(k[0] + 0x9E3779B9) & 0xFFFFFFFF, (k[1] + 0xBB67AE85) & 0xFFFFFFFF]
+    return c
+
+
+def test_philox_known_answers():
+    rows = [l.split() for l in open(os.path.join(GOLDEN, "philox4x32_10_kat.txt")) if l[0] not in "#\n"]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(x, 16) for x in r]
+        out = oracle.philox4x32_10(v[0:4], v[4:6])
+        assert [int(x) for x in out] == v[6:10]
+
+
+def test_philox_random_counters_match_python_restatement():
+    rng = np.random.default_rng(0)
+    for _ in range(50):
+        ctr = [int(x) for x in rng.integers(0, 2**32, 4)]
+        key = [int(x) for x in rng.integers(0, 2**32, 2)]
+        assert [int(x) for x in oracle.philox4x32_10(ctr, key)] == _py_philox(ctr, key)
+
+
+# ----------------------------------------------------------------------------- O1 kernel table
+def test_kernel_table_equals_quadrature_of_rectangle():
+    """Eq. 5-6: K[k][j] = (1/2pi) int_bin exp(-w tau_j) dw.  Non-square grid so a
+    transposed table fails."""
+    omega = np.arange(7) * 0.37          # left edges
+    tau = np.arange(5) * 0.21
+    K = oracle.kernel_table(omega, tau)
+    assert K.shape == (7, 5)
+    dw = 0.37
+    for k in range(7):
+        for j in range(5):
+            ref, _ = integrate.quad(lambda w: math.exp(-w * tau[j]) / TWO_PI, omega[k], omega[k] + dw,
+                                    epsabs=0, epsrel=2e-14)
+            assert K[k, j] == pytest.approx(ref, rel=2e-14)
+
+
+def test_c_vector_eq8_and_small_argument():
+    """Eq. 8: c_0 = dw/2pi; c_i = (1-exp(-i dw dtau))/(2pi i dtau).  At small x the
+    expm1 form (reading G2) must agree with the series to full precision."""
+    omega = np.arange(16) * 0.005859375
+    tau = np.array([0.0, 0.01, 0.02, 5.11])
+    c = oracle.cvec(omega, tau)
+    dw = 0.005859375
+    assert c[0] == pytest.approx(dw / TWO_PI, rel=1e-15)
+    for j in (1, 2, 3):
+        x = dw * tau[j]
+        series = (dw / TWO_PI) * (1 - x / 2 + x * x / 6 - x**3 / 24 + x**4 / 120 - x**5 / 720)
+        assert c[j] == pytest.approx(series, rel=3e-15)
+
+
+def test_flat_spectrum_closed_form_and_eq16():
+    """a == 1 on [0, w_max]: M(tau) = (1 - exp(-w_max tau))/(2 pi tau); Eq. 16: M(0) = c_0 A."""
+    n_omega, w_max = 40, 5.0
+    omega = np.arange(n_omega) * (w_max / n_omega)
+    tau = np.arange(9) * 0.3
+    K = oracle.kernel_table(omega, tau)
+    M = oracle.forward(K, np.ones(n_omega))
+    ref = np.where(tau > 0, -np.expm1(-w_max * np.maximum(tau, 1e-300)) / (TWO_PI * np.maximum(tau, 1e-300)),
+                   w_max / TWO_PI)
+    np.testing.assert_allclose(M, ref, rtol=1e-14)
+    a = np.random.default_rng(1).random(n_omega)
+    assert oracle.forward(K, a)[0] == pytest.approx((w_max / n_omega) / TWO_PI * a.sum(), rel=1e-15)
+
+
+# ----------------------------------------------------------------------------- O2 forward
+def test_forward_matches_longdouble_piecewise_integral():
+    """Eq. 5: the model is the exact integral of the piecewise-constant function —
+    evaluated here bin by bin in extended precision without the c_j q^{ij} factorisation."""
+    omega = np.arange(64) * 0.125
+    tau = np.arange(32) * 0.05
+    a = wl.bin_averages(omega, 0.125)
+    M = oracle.forward(oracle.kernel_table(omega, tau), a)
+    al, ol = a.astype(np.longdouble), omega.astype(np.longdouble)
+    dw = np.longdouble(0.125)
+    two_pi = 2 * np.longdouble(np.pi) + np.longdouble(2.4492935982947064e-16)  # pi to ~1e-32
+    for j, t in enumerate(tau.astype(np.longdouble)):
+        if t == 0:
+            ref = (al * dw).sum() / two_pi
+        else:
+            ref = (al * (np.exp(-ol * t) - np.exp(-(ol + dw) * t)) / t).sum() / two_pi
+        assert float(abs(M[j] - ref) / ref) < 1e-13
+
+
+def test_forward_converges_to_simpson_F_second_order():
+    """north_star check: with a = exact bin averages of the truncated double Lorentzian the model tends
+    to the 1e6-interval Simpson F with error ~ domega^2 (ratio 4 per halving)."""
+    tau = np.arange(16) * 0.1
+    F = wl.correlation_simpson(tau, 1_000_000)
+    errs = []
+    for n in (256, 512, 1024, 2048):
+        dw = 8.0 / n
+        omega = np.arange(n) * dw
+        M = oracle.forward(oracle.kernel_table(omega, tau), wl.bin_averages(omega, dw))
+        errs.append(np.abs(M - F)[1:].max())
+        assert abs(M[0] - F[0]) < 1e-13            # tau = 0: both are (1/2pi) int S exactly
+    ratios = [errs[i] / errs[i + 1] for i in range(3)]
+    assert all(3.8 < r < 4.2 for r in ratios), ratios
+    assert errs[-1] < 1e-6
+
+
+# ----------------------------------------------------------------------------- O3 residue
+def test_chi2_brute_force_tiny_grid():
+    """Eq. 9 with sigma (G3), on a 3x4 grid where the model is integrated numerically."""
+    omega = np.array([0.0, 0.5, 1.0])
+    tau = np.array([0.0, 0.4, 0.8, 1.2])
+    a = np.array([0.3, 1.1, 0.6])
+    F = np.array([0.16, 0.11, 0.08, 0.055])
+    sigma = np.array([1e-2, 2e-2, 1e-2, 3e-2])
+    M = oracle.forward(oracle.kernel_table(omega, tau), a)
+    brute = 0.0
+    for j in range(4):
+        m = sum(integrate.quad(lambda w: a[k] * math.exp(-w * tau[j]) / TWO_PI, omega[k], omega[k] + 0.5,
+                               epsabs=0, epsrel=2e-14)[0] for k in range(3))
+        brute += ((m - F[j]) / sigma[j]) ** 2
+    assert oracle.chi2(M, F, sigma) == pytest.approx(brute, rel=1e-12)
+    assert oracle.chi2(M, F, None) == pytest.approx(((M - F) ** 2).sum(), rel=1e-14)
+
+
+# ----------------------------------------------------------------------------- O4 start
+def test_init_tilt_meets_both_sum_rules_and_is_positive():
+    for name in ("tiny", "small"):
+        w = wl.make(name, simpson_intervals=20_000)
+        a = oracle.init_tilt(w.omega, w.A, w.B)
+        wm = w.omega + 0.5 * w.domega
+        assert (a > 0).all()
+        assert a.sum() == pytest.approx(w.A, rel=1e-13)
+        assert (a * wm).sum() == pytest.approx(w.B, rel=1e-12)
+    # reduces to the flat spectrum when omega_c is the grid midpoint (G4)
+    omega = np.arange(10) * 0.2
+    a = oracle.init_tilt(omega, 5.0, 5.0 * 1.0)
+    np.testing.assert_allclose(a, 0.5, rtol=1e-12)
+    with pytest.raises(ValueError):
+        oracle.init_tilt(omega, 1.0, 100.0)
+
+
+# ----------------------------------------------------------------------------- O5 move
+def _oracle_for(w, seed=1234, **kw):
+    o = oracle.Oracle(w.omega, w.tau, w.F, w.sigma, w.A, w.B, w.eta, seed, **kw)
+    return o
+
+
+@pytest.fixture(scope="module")
+def tiny():
+    return wl.make("tiny", simpson_intervals=100_000)
+
+
+def test_move_draws_follow_the_counter_layout(tiny):
+    """Reading G14/G11/G6: ctr = (walker, sweep, move, 0); p = (x0 N)>>32, s != p; rho = 1 - y eta (2u-1)."""
+    o = _oracle_for(tiny, seed=0x1234_5678_9ABC_DEF0)
+    o.init_walkers(4)
+    for (wk, sw, mv) in [(0, 0, 0), (3, 17, 63), (2, 100000, 5)]:
+        tr = o.move(wk, sw, mv, T=1.0, y=0.5)
+        x = _py_philox([wk, sw, mv, 0], [0x9ABCDEF0, 0x12345678])
+        p = (x[0] * 64) >> 32
+        s = (x[1] * 63) >> 32
+        s += s >= p
+        assert (tr["p"], tr["s"]) == (p, s) and p != s
+        rho = 1.0 - 0.5 * tiny.eta * (2.0 * ((x[2] + 0.5) / 2**32) - 1.0)
+        assert tr["rho"] == pytest.approx(rho, rel=1e-15)
+        assert tr["ln_u"] == pytest.approx(math.log((x[3] + 0.5) / 2**32), rel=1e-15)
+
+
+def test_index_selection_uniform(tiny):
+    """Zero-length walk = uniform p and uniform s != p."""
+    o = _oracle_for(tiny)
+    o.init_walkers(1)
+    tr, _ = o.anneal(np.full(300, 1.0), trace_walkers=(0, 1))
+    p, s = tr["p"].ravel(), tr["s"].ravel()
+    assert (p != s).all() and p.min() == 0 and p.max() == 63 and s.min() == 0 and s.max() == 63
+    n = p.size
+    for v in (p, s):
+        cnt = np.bincount(v, minlength=64)
+        chi = ((cnt - n / 64) ** 2 / (n / 64)).sum()
+        assert chi < 63 + 5 * math.sqrt(2 * 63)
+    assert np.bincount((s - p) % 64, minlength=64)[0] == 0
+
+
+def test_move_preserves_both_sum_rules_and_tau0(tiny):
+    """Eq. 20-21: A and B unchanged to 1e-13 per move; Eq. 16: dM_0 = 0."""
+    o = _oracle_for(tiny)
+    o.init_walkers(8)
+    wm = tiny.omega + 0.5 * tiny.domega
+    n_acc = 0
+    for mv in range(400):
+        for wk in range(8):
+            a0, M0 = o.a[wk].copy(), o.M[wk].copy()
+            tr = o.move(wk, 0, mv, T=1e300)         # T -> inf: every feasible move is accepted
+            if tr["flags"] & 2:
+                n_acc += 1
+                assert abs(o.a[wk].sum() - a0.sum()) <= 1e-13 * a0.sum()
+                assert abs((o.a[wk] * wm).sum() - (a0 * wm).sum()) <= 1e-13 * (a0 * wm).sum()
+                assert abs(o.M[wk][0] - M0[0]) <= 4e-16 * M0[0]
+                assert (o.a[wk] >= 0).all()
+            else:
+                assert not (tr["flags"] & 1)         # at T=inf only infeasible moves are rejected
+                np.testing.assert_array_equal(o.a[wk], a0)
+                np.testing.assert_array_equal(o.M[wk], M0)
+    assert n_acc > 1000
+
+
+def test_move_is_a_homothety_about_the_two_bin_vertex(tiny):
+    """Derived from Eq. 17-21: a' - e = rho (a - e), e = two-bin spectrum carrying A and B in bins p, s."""
+    o = _oracle_for(tiny)
+    o.init_walkers(1)
+    wm = tiny.omega + 0.5 * tiny.domega
+    A, B = tiny.A, tiny.B
+    done = 0
+    for mv in range(200):
+        a0 = o.a[0].copy()
+        tr = o.move(0, 3, mv, T=1e300)
+        if not tr["flags"] & 2:
+            continue
+        p, s, rho = tr["p"], tr["s"], tr["rho"]
+        e = np.zeros_like(a0)
+        e[p] = (B - A * wm[s]) / (wm[p] - wm[s])
+        e[s] = (B - A * wm[p]) / (wm[s] - wm[p])
+        np.testing.assert_allclose(o.a[0] - e, rho * (a0 - e), rtol=0, atol=1e-12 * np.abs(e).max())
+        done += 1
+    assert done > 50
+
+
+def test_straddling_contraction_is_never_infeasible(tiny):
+    """If p, s straddle omega_c = B/A (e >= 0) and 0 < rho <= 1 the move is a convex combination
+    (PAPER.md:137-143 + homothety): positivity can never fail."""
+    o = _oracle_for(tiny)
+    o.init_walkers(1)
+    wm = tiny.omega + 0.5 * tiny.domega
+    wc = tiny.B / tiny.A
+    seen = 0
+    for sw in range(40):
+        for mv in range(64):
+            tr = o.move(0, sw, mv, T=1e-300)        # nothing uphill accepted, state nearly frozen
+            straddle = (wm[tr["p"]] - wc) * (wm[tr["s"]] - wc) < 0
+            if straddle and tr["rho"] <= 1.0:
+                assert tr["flags"] & 1
+                seen += 1
+    assert seen > 100
+
+
+def test_incremental_dchi2_equals_from_scratch(tiny):
+    """Eq. 22 with c_j (reading G1) + Eq. 9: Delta chi^2 and the updated M agree with a full recompute."""
+    o = _oracle_for(tiny)
+    o.init_walkers(2)
+    K = o.K
+    for mv in range(300):
+        wk = mv % 2
+        a0 = o.a[wk].copy()
+        c0 = oracle.chi2(oracle.forward(K, a0), tiny.F, tiny.sigma)
+        tr = o.move(wk, 1, mv, T=1e300)
+        if tr["flags"] & 2:
+            M1 = oracle.forward(K, o.a[wk])
+            c1 = oracle.chi2(M1, tiny.F, tiny.sigma)
+            np.testing.assert_allclose(o.M[wk], M1, rtol=1e-12)
+            assert abs((c1 - c0) - tr["dchi2"]) <= 1e-12 * tr["l1"] + 1e-9 * abs(tr["dchi2"])
+
+
+def test_move_brute_force_on_tiny_grid():
+    """north_star: brute-force chi^2 on tiny grids — the move's Delta chi^2 against chi^2 evaluated by
+    numerical integration of the rectangles before and after."""
+    omega = np.arange(4) * 0.6
+    tau = np.arange(3) * 0.5
+    a = np.array([0.9, 0.4, 0.7, 0.2])
+    wm = omega + 0.3
+    A, B = a.sum(), (a * wm).sum()
+    F = np.array([0.2, 0.12, 0.08])
+    sigma = np.array([0.01, 0.02, 0.015])
+
+    def brute(av):
+        tot = 0.0
+        for j in range(3):
+            m = sum(integrate.quad(lambda w: av[k] * math.exp(-w * tau[j]) / TWO_PI, omega[k], omega[k] + 0.6,
+                                   epsabs=0, epsrel=2e-14)[0] for k in range(4))
+            tot += ((m - F[j]) / sigma[j]) ** 2
+        return tot
+
+    o = oracle.Oracle(omega, tau, F, sigma, A, B, 0.3, 99)
+    o.init_walkers(1, spectra=a[None, :])
+    n = 0
+    for mv in range(30):
+        a0 = o.a[0].copy()
+        tr = o.move(0, 0, mv, T=1e300)
+        if tr["flags"] & 2:
+            assert brute(o.a[0]) - brute(a0) == pytest.approx(tr["dchi2"], rel=1e-9, abs=1e-9)
+            n += 1
+    assert n >= 10
+
+
+# ----------------------------------------------------------------------------- Metropolis (Eq. 10)
+def test_metropolis_limits(tiny):
+    o = _oracle_for(tiny)
+    o.init_walkers(4)
+    c_prev = o.chi2.copy()
+    _, flags = o.anneal(np.full(5, 1e-300), want_flags=True)     # T -> 0+: chi^2 never increases
+    assert (o.chi2 <= c_prev).all()
+    tr, flags = o.anneal(np.full(3, 1e300), trace_walkers=(0, 4), want_flags=True)  # T -> inf
+    assert ((flags & 1) * 2 == (flags & 2)).all()                  # feasible <=> accepted
+    assert (tr["flags"] == flags[:, :, :]).all()
+
+
+def test_metropolis_frequency_matches_boltzmann_factor(tiny):
+    """Acceptance frequency of uphill moves in a Delta/T bin equals exp(-Delta/T)."""
+    o = _oracle_for(tiny, amp_mode=0)
+    o.init_walkers(64)
+    o.anneal(np.full(30, 1e3))                                     # relax away from the start
+    keep = (o.a.copy(), o.M.copy(), o.chi2.copy(), o.sweep)
+    tr, _ = o.anneal(np.full(10, 1e3), trace_walkers=(0, 64))      # probe the scale of uphill moves
+    t = tr.ravel()
+    up = ((t["flags"] & 1) == 1) & (t["dchi2"] > 0)
+    T = float(np.median(t["dchi2"][up]))
+    o.a[:], o.M[:], o.chi2[:], o.sweep = keep
+    tr, _ = o.anneal(np.full(80, T), trace_walkers=(0, 64))
+    t = tr.ravel()
+    feas = (t["flags"] & 1) == 1
+    x = t["dchi2"] / T
+    for lo, hi in [(0.05, 0.15), (0.3, 0.5), (0.9, 1.1), (1.8, 2.2)]:
+        sel = feas & (x > lo) & (x < hi)
+        n = sel.sum()
+        assert n > 300, (lo, hi, n)
+        expect = np.exp(-x[sel]).mean()
+        got = ((t["flags"][sel] & 2) == 2).mean()
+        assert abs(got - expect) < 5 * math.sqrt(expect * (1 - expect) / n), (lo, hi, got, expect)
+    down = feas & (x < 0)
+    assert ((t["flags"][down] & 2) == 2).all()                     # downhill always accepted
+
+
+# ----------------------------------------------------------------------------- Eq. 30
+def test_amp_factor_eq30():
+    """y = 1 for a >= p; (a/p)^m below; p = 1, m = 2 gives y = a^2."""
+    assert oracle.amp_factor(1.0) == 1.0
+    assert oracle.amp_factor(0.5) == 0.25
+    assert oracle.amp_factor(0.25, amp_p=0.5, amp_m=3.0) == pytest.approx(0.125)
+    assert oracle.amp_factor(0.7, amp_p=0.5) == 1.0
+    assert oracle.amp_factor(0.0) == 1e-6                          # floor (G7)
+
+
+def test_sweep_updates_y_from_its_own_acceptance(tiny):
+    o = _oracle_for(tiny)
+    o.init_walkers(3)
+    _, flags = o.anneal(np.array([0.5]), want_flags=True)
+    rate = ((flags[:, 0, :] & 2) == 2).sum(axis=1) / 64.0
+    np.testing.assert_allclose(o.y, np.where(rate >= 1, 1.0, np.maximum(rate**2, 1e-6)), rtol=1e-15)
+    assert (o.acc == ((flags & 2) == 2).sum(axis=(1, 2))).all()
+
+
+# ----------------------------------------------------------------------------- resync / splitting
+def test_split_runs_and_resync_are_consistent(tiny):
+    """Absolute sweep counter: one 6-sweep call == 2+4 sweeps; resync leaves chi^2 to rounding."""
+    sched = wl.geometric_schedule(1.0, 0.1, 6)
+    o1 = _oracle_for(tiny); o1.init_walkers(4); o1.anneal(sched)
+    o2 = _oracle_for(tiny); o2.init_walkers(4); o2.anneal(sched[:2]); o2.anneal(sched[2:])
+    np.testing.assert_array_equal(o1.a, o2.a)
+    np.testing.assert_array_equal(o1.chi2, o2.chi2)
+    c = o1.chi2.copy()
+    o1.resync()
+    np.testing.assert_allclose(o1.chi2, c, rtol=1e-9)
+
+
+# ----------------------------------------------------------------------------- O8 branching
+def test_branch_multipliers_sum_to_W_and_have_mean_w(tiny):
+    """Eq. 25: E[m] = w and sum m = W for the once-generated xi set (comb, B2)."""
+    o = _oracle_for(tiny)
+    o.init_walkers(64)
+    o.anneal(np.full(3, 1.0))
+    T = float(np.std(o.chi2)) * 2.0
+    w = np.exp(-(o.chi2 - o.chi2.min()) / T)
+    w *= 64 / w.sum()
+    acc = np.zeros(64)
+    a_keep, M_keep, c_keep = o.a.copy(), o.M.copy(), o.chi2.copy()
+    n_ev = 400
+    for ev in range(n_ev):
+        o.a[:], o.M[:], o.chi2[:] = a_keep, M_keep, c_keep
+        o.sweep = 1000 + ev                                       # xi depends on the sweep counter
+        n_rec, mult, donor = o.branch(T, 0.0)                     # t = 0: state untouched
+        assert mult.sum() == 64
+        assert ((mult == np.floor(w)) | (mult == np.ceil(w)) | (np.abs(mult - w) < 1 + 1e-9)).all()
+        assert n_rec == (mult == 0).sum() == np.maximum(mult - 1, 0).sum()
+        acc += mult
+        np.testing.assert_array_equal(o.a, a_keep)                # t = 0 is a no-op (Eq. 26)
+    np.testing.assert_allclose(acc / n_ev, w, atol=5 * 0.5 / math.sqrt(n_ev) + 1e-9)
+
+
+def test_branch_imprint_t1_copies_and_t_preserves_sum_rules(tiny):
+    """Eq. 26: t = 1 is classic branching (recipient == donor); any t keeps A, B
+    (linearity); donors unchanged; chi^2 of recipients recomputed from their new spectrum."""
+    wm = tiny.omega + 0.5 * tiny.domega
+    for t in (1.0, 0.1):
+        o = _oracle_for(tiny)
+        o.init_walkers(64)
+        o.anneal(np.full(3, 1.0))
+        a0 = o.a.copy()
+        n_rec, mult, donor = o.branch(float(np.std(o.chi2)), t)
+        assert n_rec > 0
+        rec = np.where(donor >= 0)[0]
+        assert (mult[rec] == 0).all() and (mult[donor[rec]] >= 2).all()
+        # each donor serves exactly m-1 recipients, recipients in ascending order get ascending donors
+        assert (np.bincount(donor[rec], minlength=64) == np.maximum(mult - 1, 0)).all()
+        assert (np.diff(donor[rec]) >= 0).all()
+        others = np.where(donor < 0)[0]
+        np.testing.assert_array_equal(o.a[others], a0[others])
+        for i in rec:
+            if t == 1.0:
+                np.testing.assert_array_equal(o.a[i], a0[donor[i]])
+            np.testing.assert_allclose(o.a[i], t * a0[donor[i]] + (1 - t) * a0[i], rtol=1e-15)
+            assert o.a[i].sum() == pytest.approx(tiny.A, rel=1e-13)
+            assert (o.a[i] * wm).sum() == pytest.approx(tiny.B, rel=1e-12)
+            M = oracle.forward(o.K, o.a[i])
+            np.testing.assert_array_equal(o.M[i], M)
+            assert o.chi2[i] == oracle.chi2(M, tiny.F, tiny.sigma)
