@@ -1,0 +1,193 @@
+/*
+ * sail.h — C ABI of sail-b200: the B200 (sm_100a) hot path of SAIL, "simulated annealing for the
+ * inverse Laplace transform" (arXiv 1609.07936; citations are /root/reference/PAPER.md:<line>).
+ *
+ * The calls follow the paper's problem statement (inputs N_tau, dtau, F~; omega_max, N_omega; B —
+ * PAPER.md:214, :127) and BASELINE.json's north_star list:
+ *     sail_create -> sail_init_walkers -> { sail_anneal | sail_branch | sail_resync }* -> sail_get
+ *     -> sail_destroy.
+ * Every step of the path runs in hand-written CUDA kernels; there is no CPU fallback: without a
+ * usable CUDA device every call returns SAIL_ERR_CUDA.
+ *
+ * Conventions
+ *   - plain C types only; "host" / "device" is stated for every pointer.
+ *   - all functions return a status code (0 = SAIL_OK, negative = error); no exception crosses the
+ *     boundary; sail_last_error() gives the text of the last error of a handle (or of create).
+ *   - one handle = one CUDA stream = one thread at a time; no global state.
+ *   - all floating point is IEEE binary64 ("fp64"); matrices are row-major, contiguous.
+ *   - work is enqueued on the handle's stream; calls that copy to HOST memory synchronise it.
+ *
+ * Method summary (notation of DESIGN.md §1):
+ *   spectrum of a walker: a_k >= 0 on bins [omega_k, omega_k + domega), k = 0..N_omega-1 (Eq. 3, :65)
+ *   model:   M_j = sum_k a_k K_kj,  K_kj = c_j exp(-omega_k tau_j)  (Eq. 5-8, :75-88)
+ *   residue: chi^2 = sum_j ((M_j - F_j)/sigma_j)^2                  (Eq. 9, :92, with error bars)
+ *   sums:    A = sum_k a_k,  B = sum_k a_k (omega_k + domega/2)      (Eq. 12-15, :111-121)
+ */
+#ifndef SAIL_B200_H
+#define SAIL_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SAIL_ABI_VERSION 1
+
+/* every function below is exported with default visibility; everything else in the library is hidden */
+#if defined(__GNUC__)
+#define SAIL_API __attribute__((visibility("default")))
+#else
+#define SAIL_API
+#endif
+
+enum {
+    SAIL_OK        = 0,
+    SAIL_ERR_ARG   = -1,  /* NULL / out-of-range argument, unsupported size                       */
+    SAIL_ERR_GRID  = -2,  /* omega or tau grid not uniform (rel. deviation > 1e-12) or not ascending */
+    SAIL_ERR_ALLOC = -3,  /* workspace too small / device allocation failed                       */
+    SAIL_ERR_CUDA  = -4,  /* no device, or a CUDA runtime error (text in sail_last_error)          */
+    SAIL_ERR_STATE = -5   /* call order violated (e.g. anneal before init_walkers)               */
+};
+
+typedef struct sail_handle sail_t;
+
+/* Device / memory configuration of a handle. */
+typedef struct {
+    int32_t device;           /* CUDA device ordinal                                               */
+    int32_t reserved;
+    void   *stream;           /* cudaStream_t to enqueue on (e.g. torch's current stream); NULL = default stream */
+    void   *workspace;        /* DEVICE pointer to caller-owned scratch (e.g. a torch uint8 tensor),
+                                 256-byte aligned, or NULL: the library then cudaMallocs its own   */
+    size_t  workspace_bytes;  /* size of workspace; must be >= sail_workspace_bytes(...)           */
+    int64_t max_walkers;      /* capacity W_max the handle is sized for                            */
+} sail_config;
+
+/* Bytes of device memory a handle needs for (n_omega, n_tau, max_walkers). */
+SAIL_API size_t sail_workspace_bytes(int32_t n_omega, int32_t n_tau, int64_t max_walkers);
+
+/*
+ * sail_create — define the inverse problem (N_tau, dtau, F~, omega_max, N_omega).
+ *   omega  HOST [n_omega]  bin LEFT edges omega_k = omega_0 + k domega, uniform, omega_0 >= 0 (Eq. 3)
+ *   tau    HOST [n_tau]    tau_j = tau_0 + j dtau, uniform, tau_0 >= 0 (Eq. 2, :61)
+ *   F      HOST [n_tau]    correlation data F~(tau_j)
+ *   sigma  HOST [n_tau]    error bars > 0, or NULL for sigma = 1 (the paper's unweighted Eq. 9)
+ * Inputs are copied; the caller keeps ownership.  Builds the device tables (c_j, exp(-omega_k tau_j),
+ * weights (c_j/sigma_j)^2).  Limits of this version: 2 <= n_omega <= 8192, 1 <= n_tau <= 512.
+ * Errors: SAIL_ERR_ARG, SAIL_ERR_GRID (the method is defined on uniform grids only, Eq. 2-3, 7),
+ * SAIL_ERR_ALLOC, SAIL_ERR_CUDA.  *out is NULL on error.
+ */
+SAIL_API int sail_create(sail_t **out, const double *omega, int32_t n_omega, const double *tau, int32_t n_tau,
+                const double *F, const double *sigma, const sail_config *cfg);
+
+/*
+ * sail_init_walkers — start W Markov walkers with sum constants A, B (Eq. 12-16).
+ *   mode 0: every walker = the exponential-tilt spectrum a_k ~ exp(-lambda omega_k^m) that meets both
+ *           sum rules (reading G4; the paper does not say how walkers start); spectra ignored.
+ *   mode 1: spectra HOST [W][n_omega] given by the caller (must be >= 0; sums are NOT re-normalised;
+ *           A and B are the constants the moves will preserve).
+ *   seed:   Philox4x32-10 key for all later random draws of this handle.
+ * Computes M, chi^2; resets the absolute sweep counter to 0, y = 1, counters = 0.
+ * Errors: SAIL_ERR_ARG (W < 1 or > max_walkers, B/A outside the grid, negative input).
+ */
+SAIL_API int sail_init_walkers(sail_t *h, int64_t W, double A, double B, uint64_t seed, int32_t mode,
+                      const double *spectra);
+
+/* One traced move (parity tests): written by sail_anneal for walkers in [trace_lo, trace_hi). */
+typedef struct {
+    int32_t p, s;            /* updated bins (Eq. 17-18)                                           */
+    int32_t flags;           /* bit0 feasible (positivity passed, :143), bit1 accepted, bit2 dchi2 evaluated */
+    int32_t move;            /* move index within the sweep                                        */
+    double  rho;             /* the paper's random scale factor r of Eq. 17-19                     */
+    double  delta_p, delta_s;/* Eq. 20-21                                                          */
+    double  dchi2;           /* incremental Delta chi^2 (valid if bit2)                            */
+    double  thr;             /* acceptance threshold -T ln(u_acc): accepted iff feasible && dchi2 < thr */
+    double  ap_new, as_new;  /* rho a_p + delta_p, rho a_s + delta_s                               */
+} sail_trace_rec;
+
+/* Parameters of sail_anneal. */
+typedef struct {
+    double  eta;             /* base amplitude: rho = 1 - y eta (2u - 1), requires 0 < eta < 1 (reading G6) */
+    int32_t amp_mode;        /* 0: y = 1;  1: Eq. 30 from the previous sweep's acceptance  */
+    int32_t lanes_per_walker;/* 0 = auto; else 8, 16 or 32 lanes of a warp cooperate on one walker  */
+    double  amp_p, amp_m;    /* Eq. 30 parameters (paper: p = 1, m = 2, :222)                      */
+    double  y_min;           /* floor of y (reading G7), e.g. 1e-6                                  */
+    int64_t resync_every;    /* full-residual resync after every such absolute sweep; 0 = never    */
+    int64_t trace_lo, trace_hi;  /* walkers whose moves are traced; lo == hi: none                 */
+    sail_trace_rec *trace;   /* DEVICE [(hi-lo)][n_sweeps][n_omega] or NULL                        */
+    uint8_t *flags;          /* DEVICE [W][n_sweeps][n_omega] per-move flag bytes, or NULL         */
+} sail_anneal_params;
+
+/*
+ * sail_anneal — n_sweeps sweeps ("macroupdates", :148, :218) of N_omega attempted moves per walker:
+ * proposal (uniform p, s != p; rho; Eq. 20-21), positivity rejection (:143), incremental
+ * Delta chi^2 over all tau (Eq. 22 + Eq. 9), Metropolis acceptance at T (Eq. 10), Eq. 30 update of
+ * y after each sweep.  T_schedule HOST [n_sweeps]: temperature of sweep (sweep_counter + i).  The
+ * absolute sweep counter continues across calls, so splitting a run does not change the random
+ * stream (Philox counter = (walker, sweep, move, 0)).  Asynchronous on the stream.
+ */
+SAIL_API int sail_anneal(sail_t *h, const double *T_schedule, int64_t n_sweeps, const sail_anneal_params *p);
+
+/* Results of one branching event. */
+typedef struct {
+    int64_t n_recipients;    /* walkers with multiplier 0 that were imprinted                      */
+    int32_t max_multiplier;
+    int32_t reserved;
+    double  chi2_min;
+} sail_branch_info;
+
+/*
+ * sail_branch — one imprinted-branching event (Eq. 24-26, :166-182; readings B1-B5):
+ * weights exp(-(chi^2 - chi^2_min)/T) normalised to W, integer multipliers by a comb over the
+ * fixed-point prefix sum (sum m = W exactly), recipients (m = 0) take t*donor + (1-t)*self for
+ * spectrum and model, their chi^2 is recomputed.  mult_out HOST [W] int32 or NULL; donor_out HOST
+ * [W] int64 (-1 for non-recipients) or NULL; info HOST or NULL.  Synchronises the stream when any
+ * output is requested.
+ */
+SAIL_API int sail_branch(sail_t *h, double T, double t_imprint, sail_branch_info *info, int32_t *mult_out,
+                int64_t *donor_out);
+
+/* sail_resync — recompute M = a K (dense W x N_omega x N_tau contraction) and chi^2 for all walkers. */
+SAIL_API int sail_resync(sail_t *h);
+
+/*
+ * sail_get — copy results out.  spectra [W][n_omega] (true coefficients a_k), chi2 [W]; either may
+ * be NULL.  on_device = 0: HOST destinations (synchronises); 1: DEVICE destinations (stream-ordered).
+ */
+SAIL_API int sail_get(sail_t *h, double *spectra, double *chi2, int32_t on_device);
+
+/* sail_get_model — M [W][n_tau] (the model correlation of each walker), HOST or DEVICE as above. */
+SAIL_API int sail_get_model(sail_t *h, double *M, int32_t on_device);
+
+/* sail_stats — HOST outputs [W], any may be NULL: accepted / evaluated move totals since init, y. */
+SAIL_API int sail_stats(sail_t *h, int64_t *accepted, int64_t *evaluated, double *y);
+
+/*
+ * sail_set_walkers — state injection for sampled parity on big configs: overwrite walkers
+ * [w0, w0+n) with HOST spectra [n][n_omega] and (optionally, may be NULL) HOST y [n]; M and chi^2
+ * are recomputed.  sail_set_sweep sets the absolute sweep counter.
+ */
+SAIL_API int sail_set_walkers(sail_t *h, int64_t w0, int64_t n, const double *spectra, const double *y);
+SAIL_API int sail_set_sweep(sail_t *h, int64_t sweep);
+
+/* sail_destroy — free library-owned memory (never the caller's workspace).  NULL is OK. */
+SAIL_API int sail_destroy(sail_t *h);
+
+/* Text of the last error on this handle; h == NULL: last error of sail_create in this thread. */
+SAIL_API const char *sail_last_error(const sail_t *h);
+
+/* Number of kernel launches issued by this handle so far (bench.py's gpu_launches). */
+SAIL_API int64_t sail_launch_count(const sail_t *h);
+
+/*
+ * Diagnostics used by bench.py for the roofline denominators (not part of the method):
+ * sail_measure_fp64_peak — runs a register-resident DFMA microbenchmark on `device`, returns
+ * achieved FP64 lane-instructions per second (fused multiply-adds per second) in *dfma_per_s.
+ */
+SAIL_API int sail_measure_fp64_peak(int32_t device, void *stream, double *dfma_per_s);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SAIL_B200_H */

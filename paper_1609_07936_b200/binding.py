@@ -1,0 +1,235 @@
+"""Thin ctypes binding of libsail_b200.so (include/sail.h) — argument marshalling only.
+
+Every numerical step runs in the library's CUDA kernels.  PyTorch is used for device memory (the
+workspace and trace buffers are torch tensors) and for the stream.  There is NO fallback: if the
+shared library is missing or no CUDA device is visible, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libsail_b200.so")
+
+SAIL_OK, SAIL_ERR_ARG, SAIL_ERR_GRID, SAIL_ERR_ALLOC, SAIL_ERR_CUDA, SAIL_ERR_STATE = 0, -1, -2, -3, -4, -5
+
+EXPORTS = ["sail_workspace_bytes", "sail_create", "sail_init_walkers", "sail_anneal", "sail_branch",
+           "sail_resync", "sail_get", "sail_get_model", "sail_stats", "sail_set_walkers", "sail_set_sweep",
+           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak"]
+
+
+class SailError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"sail error {code}: {msg}")
+        self.code = code
+
+
+class sail_config(C.Structure):
+    _fields_ = [("device", C.c_int32), ("reserved", C.c_int32), ("stream", C.c_void_p),
+                ("workspace", C.c_void_p), ("workspace_bytes", C.c_size_t), ("max_walkers", C.c_int64)]
+
+
+class sail_anneal_params(C.Structure):
+    _fields_ = [("eta", C.c_double), ("amp_mode", C.c_int32), ("lanes_per_walker", C.c_int32),
+                ("amp_p", C.c_double), ("amp_m", C.c_double), ("y_min", C.c_double),
+                ("resync_every", C.c_int64), ("trace_lo", C.c_int64), ("trace_hi", C.c_int64),
+                ("trace", C.c_void_p), ("flags", C.c_void_p)]
+
+
+class sail_branch_info(C.Structure):
+    _fields_ = [("n_recipients", C.c_int64), ("max_multiplier", C.c_int32), ("reserved", C.c_int32),
+                ("chi2_min", C.c_double)]
+
+
+TRACE_DTYPE = np.dtype([("p", "<i4"), ("s", "<i4"), ("flags", "<i4"), ("move", "<i4"),
+                        ("rho", "<f8"), ("delta_p", "<f8"), ("delta_s", "<f8"), ("dchi2", "<f8"),
+                        ("thr", "<f8"), ("ap_new", "<f8"), ("as_new", "<f8")])
+
+_lib = None
+
+
+def lib():
+    """Load libsail_b200.so; raises if it has not been built (python -m paper_1609_07936_b200.build)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: build it with `python -m paper_1609_07936_b200.build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.sail_workspace_bytes.restype = C.c_size_t
+        L.sail_workspace_bytes.argtypes = [C.c_int32, C.c_int32, C.c_int64]
+        L.sail_create.argtypes = [C.POINTER(C.c_void_p), C.c_void_p, C.c_int32, C.c_void_p, C.c_int32,
+                                  C.c_void_p, C.c_void_p, C.POINTER(sail_config)]
+        L.sail_init_walkers.argtypes = [C.c_void_p, C.c_int64, C.c_double, C.c_double, C.c_uint64, C.c_int32, C.c_void_p]
+        L.sail_anneal.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(sail_anneal_params)]
+        L.sail_branch.argtypes = [C.c_void_p, C.c_double, C.c_double, C.POINTER(sail_branch_info), C.c_void_p, C.c_void_p]
+        L.sail_resync.argtypes = [C.c_void_p]
+        L.sail_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32]
+        L.sail_get_model.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
+        L.sail_stats.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
+        L.sail_set_walkers.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
+        L.sail_set_sweep.argtypes = [C.c_void_p, C.c_int64]
+        L.sail_destroy.argtypes = [C.c_void_p]
+        L.sail_last_error.restype = C.c_char_p
+        L.sail_last_error.argtypes = [C.c_void_p]
+        L.sail_launch_count.restype = C.c_int64
+        L.sail_launch_count.argtypes = [C.c_void_p]
+        L.sail_measure_fp64_peak.argtypes = [C.c_int32, C.c_void_p, C.POINTER(C.c_double)]
+        _lib = L
+    return _lib
+
+
+def _f64(x):
+    return np.ascontiguousarray(x, dtype=np.float64)
+
+
+def _ptr(arr):
+    return arr.ctypes.data_as(C.c_void_p) if arr is not None else None
+
+
+def measure_fp64_peak(device=0):
+    """FP64 fused multiply-adds per second (lane-instructions/s) of a register-resident DFMA loop."""
+    import torch
+    out = C.c_double(0.0)
+    rc = lib().sail_measure_fp64_peak(device, C.c_void_p(torch.cuda.current_stream(device).cuda_stream), C.byref(out))
+    if rc:
+        raise SailError(rc, lib().sail_last_error(None).decode())
+    return out.value
+
+
+class Sail:
+    """One inverse problem + its walker population on one GPU (handle of include/sail.h)."""
+
+    def __init__(self, omega, tau, F, sigma=None, max_walkers=1, device=0, torch_workspace=True):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("sail-b200 needs a CUDA device; there is no CPU fallback")
+        L = lib()
+        self._L = L
+        self.device = device
+        omega, tau, F = _f64(omega), _f64(tau), _f64(F)
+        sg = _f64(sigma) if sigma is not None else None
+        self.n_omega, self.n_tau = omega.size, tau.size
+        self.max_walkers = int(max_walkers)
+        cfg = sail_config()
+        cfg.device = device
+        cfg.stream = torch.cuda.current_stream(device).cuda_stream
+        cfg.max_walkers = self.max_walkers
+        self._ws = None
+        if torch_workspace:
+            nbytes = L.sail_workspace_bytes(self.n_omega, self.n_tau, self.max_walkers)
+            self._ws = torch.empty(nbytes + 256, dtype=torch.uint8, device=f"cuda:{device}")
+            base = (self._ws.data_ptr() + 255) & ~255
+            cfg.workspace = base
+            cfg.workspace_bytes = nbytes
+        h = C.c_void_p()
+        rc = L.sail_create(C.byref(h), _ptr(omega), self.n_omega, _ptr(tau), self.n_tau, _ptr(F), _ptr(sg), C.byref(cfg))
+        if rc:
+            raise SailError(rc, L.sail_last_error(None).decode())
+        self._h = h
+        self.W = 0
+
+    # ------------------------------------------------------------------------------------------
+    def _check(self, rc):
+        if rc:
+            raise SailError(rc, self._L.sail_last_error(self._h).decode())
+
+    def init_walkers(self, W, A, B, seed, spectra=None):
+        sp = _f64(spectra) if spectra is not None else None
+        if sp is not None and sp.size != W * self.n_omega:
+            raise ValueError("spectra must be [W][n_omega]")
+        self._check(self._L.sail_init_walkers(self._h, W, A, B, C.c_uint64(seed), 0 if sp is None else 1, _ptr(sp)))
+        self.W = W
+
+    def anneal(self, T_schedule, eta, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6, resync_every=0,
+               lanes_per_walker=0, trace_walkers=None, want_flags=False):
+        """Run len(T_schedule) sweeps.  Returns (trace, flags) numpy arrays when requested, else (None, None)."""
+        import torch
+        T = _f64(T_schedule)
+        p = sail_anneal_params()
+        p.eta, p.amp_mode, p.lanes_per_walker = eta, amp_mode, lanes_per_walker
+        p.amp_p, p.amp_m, p.y_min, p.resync_every = amp_p, amp_m, y_min, resync_every
+        trace_t = flags_t = None
+        if trace_walkers is not None:
+            lo, hi = trace_walkers
+            p.trace_lo, p.trace_hi = lo, hi
+            nbytes = (hi - lo) * T.size * self.n_omega * TRACE_DTYPE.itemsize
+            trace_t = torch.zeros(nbytes, dtype=torch.uint8, device=f"cuda:{self.device}")
+            p.trace = trace_t.data_ptr()
+        if want_flags:
+            flags_t = torch.zeros(self.W * T.size * self.n_omega, dtype=torch.uint8, device=f"cuda:{self.device}")
+            p.flags = flags_t.data_ptr()
+        self._check(self._L.sail_anneal(self._h, _ptr(T), T.size, C.byref(p)))
+        trace = flags = None
+        if trace_t is not None:
+            lo, hi = trace_walkers
+            trace = trace_t.cpu().numpy().view(TRACE_DTYPE).reshape(hi - lo, T.size, self.n_omega)
+        if flags_t is not None:
+            flags = flags_t.cpu().numpy().reshape(self.W, T.size, self.n_omega)
+        return trace, flags
+
+    def branch(self, T, t_imprint, want_maps=False):
+        info = sail_branch_info()
+        mult = np.empty(self.W, dtype=np.int32) if want_maps else None
+        donor = np.empty(self.W, dtype=np.int64) if want_maps else None
+        self._check(self._L.sail_branch(self._h, T, t_imprint, C.byref(info), _ptr(mult), _ptr(donor)))
+        return info, mult, donor
+
+    def branch_async(self, T, t_imprint):
+        self._check(self._L.sail_branch(self._h, T, t_imprint, None, None, None))
+
+    def resync(self):
+        self._check(self._L.sail_resync(self._h))
+
+    def get(self, spectra=True, chi2=True):
+        sp = np.empty((self.W, self.n_omega)) if spectra else None
+        c2 = np.empty(self.W) if chi2 else None
+        self._check(self._L.sail_get(self._h, _ptr(sp), _ptr(c2), 0))
+        return sp, c2
+
+    def get_into(self, spectra_host, chi2_host):
+        """Copy into caller-provided (e.g. pinned) host arrays."""
+        self._check(self._L.sail_get(self._h, _ptr(spectra_host), _ptr(chi2_host), 0))
+
+    def get_device(self, spectra_t=None, chi2_t=None):
+        """Stream-ordered copy into torch CUDA tensors (float64)."""
+        self._check(self._L.sail_get(self._h, spectra_t.data_ptr() if spectra_t is not None else None,
+                                     chi2_t.data_ptr() if chi2_t is not None else None, 1))
+
+    def get_model(self):
+        M = np.empty((self.W, self.n_tau))
+        self._check(self._L.sail_get_model(self._h, _ptr(M), 0))
+        return M
+
+    def stats(self):
+        acc = np.empty(self.W, dtype=np.int64)
+        ev = np.empty(self.W, dtype=np.int64)
+        y = np.empty(self.W)
+        self._check(self._L.sail_stats(self._h, _ptr(acc), _ptr(ev), _ptr(y)))
+        return acc, ev, y
+
+    def set_walkers(self, w0, spectra, y=None):
+        sp = _f64(spectra).reshape(-1, self.n_omega)
+        yy = _f64(y) if y is not None else None
+        self._check(self._L.sail_set_walkers(self._h, w0, sp.shape[0], _ptr(sp), _ptr(yy)))
+
+    def set_sweep(self, sweep):
+        self._check(self._L.sail_set_sweep(self._h, sweep))
+
+    def launch_count(self):
+        return int(self._L.sail_launch_count(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None):
+            self._L.sail_destroy(self._h)
+            self._h = None
+        self._ws = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,234 @@
+// branch.cu — imprinted branching (Eq. 24-26; readings B1-B5 in
+// DESIGN.md §2): fixed-point weights -> integer prefix sum -> comb multipliers (sum m = W exactly) ->
+// donor map by binary search -> coalesced 128-bit imprint copy of (spectrum, model) + residue.
+#include "sail_internal.cuh"
+
+namespace sail {
+
+constexpr int kScanThreads = 256;
+constexpr int kScanItems = 4;
+constexpr int kScanTile = kScanThreads * kScanItems;   // 1024 elements per CTA
+
+__global__ void chi2_min_kernel(long long W, const double *__restrict__ chi2, unsigned long long *scalars)
+{
+    // chi^2 >= 0, so the IEEE bit patterns order like the values
+    unsigned long long m = ~0ull;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
+        const unsigned long long b = (unsigned long long)__double_as_longlong(chi2[i]);
+        m = b < m ? b : m;
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const unsigned long long o = __shfl_xor_sync(0xffffffffu, m, off);
+        m = o < m ? o : m;
+    }
+    if ((threadIdx.x & 31) == 0) atomicMin(scalars + 0, m);
+}
+
+// B1 + B3: e_i = exp(-(chi2_i - chi2_min)/T), E_i = floor(e_i 2^40)
+__global__ void weights_kernel(long long W, const double *__restrict__ chi2, double T,
+                               const unsigned long long *scalars, unsigned long long *ehat)
+{
+    const double cmin = __longlong_as_double((long long)scalars[0]);
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
+        const double e = exp(-(chi2[i] - cmin) / T);
+        ehat[i] = (unsigned long long)floor(e * 1099511627776.0);
+    }
+}
+
+// ---- three-phase inclusive scan of u64 arrays (blockIdx.y selects the array) -----------------------
+struct ScanArrays { unsigned long long *arr[2]; unsigned long long *sums[2]; };
+
+__global__ void __launch_bounds__(kScanThreads) scan_tiles_kernel(long long n, ScanArrays S)
+{
+    __shared__ unsigned long long warp_tot[kScanThreads / 32];
+    unsigned long long *x = S.arr[blockIdx.y];
+    const long long base = (long long)blockIdx.x * kScanTile + (long long)threadIdx.x * kScanItems;
+    unsigned long long v[kScanItems], run = 0;
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i) {
+        v[i] = (base + i < n) ? x[base + i] : 0ull;
+        run += v[i];
+        v[i] = run;
+    }
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    unsigned long long inc = run;
+#pragma unroll
+    for (int off = 1; off < 32; off <<= 1) {
+        const unsigned long long o = __shfl_up_sync(0xffffffffu, inc, off);
+        if (lane >= off) inc += o;
+    }
+    if (lane == 31) warp_tot[wid] = inc;
+    __syncthreads();
+    unsigned long long prefix = inc - run;
+    for (int w2 = 0; w2 < wid; ++w2) prefix += warp_tot[w2];
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i)
+        if (base + i < n) x[base + i] = v[i] + prefix;
+    if (threadIdx.x == kScanThreads - 1) S.sums[blockIdx.y][blockIdx.x] = prefix + run;
+}
+
+__global__ void scan_sums_kernel(int n_tiles, ScanArrays S)
+{
+    // few tiles (W/1024): one thread per array is enough and keeps the result exact and ordered
+    if (threadIdx.x == 0) {
+        unsigned long long *s = S.sums[blockIdx.x];
+        unsigned long long run = 0;
+        for (int i = 0; i < n_tiles; ++i) { const unsigned long long t = s[i]; s[i] = run; run += t; }
+    }
+}
+
+__global__ void __launch_bounds__(kScanThreads) scan_add_kernel(long long n, ScanArrays S)
+{
+    unsigned long long *x = S.arr[blockIdx.y];
+    const unsigned long long off = S.sums[blockIdx.y][blockIdx.x];
+    const long long base = (long long)blockIdx.x * kScanTile + (long long)threadIdx.x * kScanItems;
+#pragma unroll
+    for (int i = 0; i < kScanItems; ++i)
+        if (base + i < n) x[base + i] += off;
+}
+
+static int scan_inclusive(sail_handle *h, long long n, int n_arrays, unsigned long long *a0, unsigned long long *a1)
+{
+    const int tiles = (int)((n + kScanTile - 1) / kScanTile);
+    ScanArrays S;
+    S.arr[0] = a0; S.arr[1] = a1;
+    S.sums[0] = h->br.block_sums; S.sums[1] = h->br.block_sums + tiles;
+    scan_tiles_kernel<<<dim3(tiles, n_arrays), kScanThreads, 0, h->stream>>>(n, S);
+    SAIL_LAUNCH_OK(h, "scan_tiles_kernel");
+    if (tiles > 1) {
+        scan_sums_kernel<<<n_arrays, 32, 0, h->stream>>>(tiles, S);
+        SAIL_LAUNCH_OK(h, "scan_sums_kernel");
+        scan_add_kernel<<<dim3(tiles, n_arrays), kScanThreads, 0, h->stream>>>(n, S);
+        SAIL_LAUNCH_OK(h, "scan_add_kernel");
+    }
+    return SAIL_OK;
+}
+
+// B2: comb multipliers m_i = floor((C_i W + Xi)/S) - floor((C_{i-1} W + Xi)/S), Xi = (x0 S) >> 32
+__global__ void multipliers_kernel(long long W, const unsigned long long *__restrict__ Cinc, uint32_t seed_lo,
+                                   uint32_t seed_hi, uint32_t sweep, int32_t *mult, unsigned long long *is_rec,
+                                   unsigned long long *extras, unsigned long long *scalars)
+{
+    const unsigned long long S = Cinc[W - 1];
+    uint32_t x[4];
+    philox4x32_10(0u, sweep, 0u, 1u, seed_lo, seed_hi, x);
+    const unsigned __int128 Xi = ((unsigned __int128)x[0] * S) >> 32;
+    int mmax = 0;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
+        const unsigned long long cprev = i ? Cinc[i - 1] : 0ull;
+        const unsigned long long hi = (unsigned long long)(((unsigned __int128)Cinc[i] * (unsigned long long)W + Xi) / S);
+        const unsigned long long lo = (unsigned long long)(((unsigned __int128)cprev * (unsigned long long)W + Xi) / S);
+        const int m = (int)(hi - lo);
+        mult[i] = m;
+        is_rec[i] = (m == 0) ? 1ull : 0ull;
+        extras[i] = (m > 1) ? (unsigned long long)(m - 1) : 0ull;
+        mmax = m > mmax ? m : mmax;
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const int o = __shfl_xor_sync(0xffffffffu, mmax, off);
+        mmax = o > mmax ? o : mmax;
+    }
+    if ((threadIdx.x & 31) == 0) atomicMax(scalars + 3, (unsigned long long)mmax);
+    if (blockIdx.x == 0 && threadIdx.x == 0) scalars[1] = S;
+}
+
+// B4: recipient of rank r takes the donor with X_i <= r < X_i + x_i (binary search on the inclusive scan)
+__global__ void donor_map_kernel(long long W, const int32_t *__restrict__ mult, const unsigned long long *__restrict__ rec_inc,
+                                 const unsigned long long *__restrict__ ext_inc, int64_t *donor_of, int64_t *rec_list,
+                                 unsigned long long *scalars)
+{
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
+        long long donor = -1;
+        if (mult[i] == 0) {
+            const unsigned long long r = rec_inc[i] - 1;
+            long long lo = 0, hi = W - 1;            // first index with ext_inc > r
+            while (lo < hi) {
+                const long long mid = (lo + hi) >> 1;
+                if (ext_inc[mid] > r) hi = mid; else lo = mid + 1;
+            }
+            donor = lo;
+            rec_list[r] = i;
+        }
+        donor_of[i] = donor;
+        if (i == W - 1) scalars[2] = rec_inc[i];
+    }
+}
+
+// Eq. 26: a(l1) <- t a(l2) + (1-t) a(l1) for spectrum and model (linearity); chi^2 of the
+// recipient from its new model.  One CTA per recipient, 128-bit accesses when rows are 16-byte aligned.
+__global__ void __launch_bounds__(256) imprint_kernel(int n_omega, int n_tau, double t, const int64_t *__restrict__ rec_list,
+                                                      const int64_t *__restrict__ donor_of, const unsigned long long *scalars,
+                                                      double *a, double *mt, double *chi2,
+                                                      const double *__restrict__ Wj, const double *__restrict__ fj)
+{
+    __shared__ double red[8];
+    const long long n_rec = (long long)scalars[2];
+    const double omt = 1.0 - t;
+    for (long long r = blockIdx.x; r < n_rec; r += gridDim.x) {
+        const long long i = rec_list[r], dn = donor_of[i];
+        double *ai = a + (size_t)i * n_omega;
+        const double *ad = a + (size_t)dn * n_omega;
+        if ((n_omega & 1) == 0) {
+            double2 *ai2 = reinterpret_cast<double2 *>(ai);
+            const double2 *ad2 = reinterpret_cast<const double2 *>(ad);
+            for (int k = threadIdx.x; k < n_omega / 2; k += blockDim.x) {
+                const double2 x = ai2[k], z = ad2[k];
+                ai2[k] = make_double2(__dadd_rn(__dmul_rn(t, z.x), __dmul_rn(omt, x.x)),
+                                      __dadd_rn(__dmul_rn(t, z.y), __dmul_rn(omt, x.y)));
+            }
+        } else {
+            for (int k = threadIdx.x; k < n_omega; k += blockDim.x)
+                ai[k] = __dadd_rn(__dmul_rn(t, ad[k]), __dmul_rn(omt, ai[k]));
+        }
+        double *mi = mt + (size_t)i * n_tau;
+        const double *md = mt + (size_t)dn * n_tau;
+        double s = 0.0;
+        for (int j = threadIdx.x; j < n_tau; j += blockDim.x) {
+            const double v = __dadd_rn(__dmul_rn(t, md[j]), __dmul_rn(omt, mi[j]));
+            mi[j] = v;
+            const double D = v - fj[j];
+            s = fma(Wj[j] * D, D, s);
+        }
+#pragma unroll
+        for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+        if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = s;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double tot = 0.0;
+            for (int w2 = 0; w2 < (int)(blockDim.x >> 5); ++w2) tot += red[w2];
+            chi2[i] = tot;
+        }
+        __syncthreads();
+    }
+}
+
+int launch_branch(sail_handle *h, double T, double t_imprint)
+{
+    const long long W = h->W;
+    BranchScratch &b = h->br;
+    const int blocks = (int)((W + 255) / 256 < 1184 ? (W + 255) / 256 : 1184);
+    SAIL_CUDA_OK(h, cudaMemsetAsync(b.scalars, 0, 8 * sizeof(unsigned long long), h->stream));
+    SAIL_CUDA_OK(h, cudaMemsetAsync(b.scalars, 0xFF, sizeof(unsigned long long), h->stream));
+    chi2_min_kernel<<<blocks, 256, 0, h->stream>>>(W, h->st.chi2, b.scalars);
+    SAIL_LAUNCH_OK(h, "chi2_min_kernel");
+    weights_kernel<<<blocks, 256, 0, h->stream>>>(W, h->st.chi2, T, b.scalars, b.ehat);
+    SAIL_LAUNCH_OK(h, "weights_kernel");
+    int rc = scan_inclusive(h, W, 1, b.ehat, nullptr);
+    if (rc) return rc;
+    multipliers_kernel<<<blocks, 256, 0, h->stream>>>(W, b.ehat, (uint32_t)(h->seed & 0xFFFFFFFFu), (uint32_t)(h->seed >> 32),
+                                                      (uint32_t)h->sweep, b.mult, b.scanA, b.scanB, b.scalars);
+    SAIL_LAUNCH_OK(h, "multipliers_kernel");
+    rc = scan_inclusive(h, W, 2, b.scanA, b.scanB);
+    if (rc) return rc;
+    donor_map_kernel<<<blocks, 256, 0, h->stream>>>(W, b.mult, b.scanA, b.scanB, b.donor_of, b.rec_list, b.scalars);
+    SAIL_LAUNCH_OK(h, "donor_map_kernel");
+    const int iblocks = (int)(W < (long long)h->num_sms * 8 ? W : (long long)h->num_sms * 8);
+    imprint_kernel<<<iblocks, 256, 0, h->stream>>>(h->n_omega, h->n_tau, t_imprint, b.rec_list, b.donor_of, b.scalars,
+                                                   h->st.a, h->st.mt, h->st.chi2, h->tab.Wj, h->tab.fj);
+    SAIL_LAUNCH_OK(h, "imprint_kernel");
+    return SAIL_OK;
+}
+
+} // namespace sail

@@ -1,0 +1,138 @@
+// sail_internal.cuh — internals of libsail_b200 (sm_100a). Not part of the ABI; see include/sail.h.
+// Shares nothing with oracle/ (the CPU oracle): tables, Philox and all arithmetic are restated here.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stdio.h>
+#include <string>
+
+#include "../../include/sail.h"
+
+namespace sail {
+
+constexpr int kMaxTau = 512;        // 32 lanes x 16 tau-points per lane (register-resident residual)
+constexpr int kMaxOmega = 8192;     // ratio + start tables + proposal records must fit 227 KB of shared memory
+constexpr int kRecBytes = 64;       // one staged proposal record in shared memory
+
+// ------------------------------------------------------------------------------------------------
+// Device-side layout of one handle.  All arrays live in ONE workspace (caller- or library-owned).
+// Residual state is kept in the "pure exponential" basis:
+//   mt_j  = M_j / c_j = sum_k a_k exp(-omega_k tau_j)          (so kernel rows are geometric in j)
+//   Wj    = (c_j / sigma_j)^2,   fj = F_j / c_j,   chi^2 = sum_j Wj (mt_j - fj)^2
+// ------------------------------------------------------------------------------------------------
+struct DevTables {
+    const double *omega;   // [n_omega] bin left edges
+    const double *tau;     // [n_tau]
+    const double *c;       // [n_tau]  Eq. 8
+    const double *Wj;      // [n_tau]
+    const double *fj;      // [n_tau]
+    const double *E;       // [n_omega][n_tau] exp(-omega_k tau_j), for the dense forward transform
+};
+
+struct DevState {
+    double *a;             // [W][n_omega] true spectral coefficients (scale folded at kernel end)
+    double *mt;            // [W][n_tau]
+    double *chi2;          // [W]
+    double *y;             // [W] Eq. 30 amplitude factor
+    unsigned long long *n_acc;   // [W] accepted moves since init
+    unsigned long long *n_eval;  // [W] feasible (evaluated) moves since init
+};
+
+struct BranchScratch {
+    unsigned long long *ehat;    // [W] fixed-point weights, then inclusive scan (in place)
+    unsigned long long *scanA;   // [W] scan of recipient flags
+    unsigned long long *scanB;   // [W] scan of donor extras
+    unsigned long long *block_sums; // [3 * kScanBlocksMax]
+    int32_t *mult;               // [W]
+    int64_t *donor_of;           // [W]
+    int64_t *rec_list;           // [W] recipient indices in ascending order
+    unsigned long long *scalars; // [8]: 0 chi2_min bits, 1 S, 2 n_rec, 3 max_mult
+};
+
+} // namespace sail
+
+struct sail_handle {
+    int device = 0;
+    cudaStream_t stream = nullptr;
+    int num_sms = 0;
+    int n_omega = 0, n_tau = 0;
+    int64_t max_walkers = 0, W = 0;
+    double omega0 = 0, domega = 0, tau0 = 0, dtau = 0;
+    double A = 0, B = 0;
+    uint64_t seed = 0;
+    int64_t sweep = 0;          // absolute sweep counter
+    bool initialised = false;
+
+    void *workspace = nullptr;  // base of everything below
+    size_t workspace_bytes = 0;
+    bool owns_workspace = false;
+
+    sail::DevTables tab{};
+    sail::DevState st{};
+    sail::BranchScratch br{};
+    // sweep-kernel tables for the lane count last used (rebuilt when it changes)
+    int tables_G = 0;
+    bool tables_fact = false;
+    int fact_shift = 0;
+    double *sw_ratio = nullptr;  // [n_omega] exp(-omega_k G dtau)
+    double *sw_E0 = nullptr;     // direct: [n_omega][G]; factored: H[n_hi][G] then L[n_lo][G]
+    double *d_T = nullptr;       // device copy of the schedule chunk (library-owned, grows)
+    size_t d_T_cap = 0;
+    double *h_pinned = nullptr;  // small pinned staging buffer
+    size_t h_pinned_cap = 0;
+
+    int64_t launches = 0;
+    std::string err;
+};
+
+namespace sail {
+
+// ---- error helpers -------------------------------------------------------------------------------
+int set_err(sail_handle *h, int code, const char *fmt, ...);
+#define SAIL_CUDA_OK(h, expr)                                                                    \
+    do {                                                                                         \
+        cudaError_t e__ = (expr);                                                                \
+        if (e__ != cudaSuccess)                                                                  \
+            return sail::set_err((h), SAIL_ERR_CUDA, "%s failed: %s (%s:%d)", #expr,             \
+                                 cudaGetErrorString(e__), __FILE__, __LINE__);                   \
+    } while (0)
+#define SAIL_LAUNCH_OK(h, what)                                                                  \
+    do {                                                                                         \
+        cudaError_t e__ = cudaGetLastError();                                                    \
+        (h)->launches++;                                                                         \
+        if (e__ != cudaSuccess)                                                                  \
+            return sail::set_err((h), SAIL_ERR_CUDA, "launch of %s failed: %s", what,            \
+                                 cudaGetErrorString(e__));                                       \
+    } while (0)
+
+// ---- Philox4x32-10 (Salmon et al. SC'11), restated for the device ---------------------------------
+__host__ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                       uint32_t k0, uint32_t k1, uint32_t (&out)[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint64_t p0 = (uint64_t)0xD2511F53u * c0;
+        const uint64_t p1 = (uint64_t)0xCD9E8D57u * c2;
+        const uint32_t n0 = (uint32_t)(p1 >> 32) ^ c1 ^ k0;
+        const uint32_t n2 = (uint32_t)(p0 >> 32) ^ c3 ^ k1;
+        c1 = (uint32_t)p1;
+        c3 = (uint32_t)p0;
+        c0 = n0;
+        c2 = n2;
+        k0 += 0x9E3779B9u;
+        k1 += 0xBB67AE85u;
+    }
+    out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
+}
+
+// ---- entry points implemented in the other translation units ---------------------------------------
+int launch_problem_tables(sail_handle *h, const double *d_F, const double *d_sigma, double *c, double *Wj,
+                          double *fj, double *E);
+int launch_forward(sail_handle *h, int64_t w0, int64_t n);            // mt, chi2 of walkers [w0, w0+n)
+int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sail_anneal_params *p,
+                  int64_t sweeps_in_call, int64_t call_offset);
+int launch_branch(sail_handle *h, double T, double t_imprint);
+int launch_scale_model(sail_handle *h, double *dst);                  // dst[w][j] = c_j mt[w][j]
+int ensure_sweep_tables(sail_handle *h, int G);
+
+} // namespace sail

@@ -1,0 +1,339 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle on the same
+seeded inputs.  Three agreement levels (BASELINE.json north_star):
+  L1  per traced move: identical p, s; rho, delta within 4 ulp; |dchi2_gpu - dchi2_cpu| <= 1e-12 * l1
+      (l1 = cancellation-aware L1 mass of the sum, computed by the oracle)
+  L2  identical accept / reject sequences, except flagged near-ties
+  L3  final spectra and chi^2 agree to 1e-9 where the sequences are identical.
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_1609_07936_b200 import workloads as wl
+
+pytestmark = pytest.mark.gpu
+
+SEED = 0x5A11_0000_0000_0001
+
+
+def _sail(w, W):
+    from paper_1609_07936_b200.binding import Sail
+    return Sail(w.omega, w.tau, w.F, w.sigma, max_walkers=W)
+
+
+def _oracle(w, W, spectra=None, seed=SEED):
+    o = oracle.Oracle(w.omega, w.tau, w.F, w.sigma, w.A, w.B, w.eta, seed)
+    o.init_walkers(W, spectra)
+    return o
+
+
+def _ulp_close(a, b, ulps=4):
+    return np.abs(a - b) <= ulps * np.spacing(np.maximum(np.abs(a), np.abs(b)))
+
+
+def compare_traces(tg, to, T_sched, stop_on_flagged=True):
+    """tg: GPU trace [nw][ns][n_omega], to: oracle trace, same shape.  Returns number of flagged near-ties."""
+    assert tg.shape == to.shape
+    assert (tg["p"] == to["p"]).all() and (tg["s"] == to["s"]).all()
+    assert (tg["move"] == to["move"]).all()
+    flagged = 0
+    for w in range(tg.shape[0]):
+        g, o = tg[w].reshape(-1), to[w].reshape(-1)
+        Tm = np.repeat(np.asarray(T_sched), tg.shape[2])
+        gacc, oacc = (g["flags"] & 3), (o["flags"] & 3)
+        mism = np.nonzero(gacc != oacc)[0]
+        end = g.size
+        if mism.size:
+            i = mism[0]
+            near_metropolis = abs(o["dchi2"][i] / Tm[i] + o["ln_u"][i]) < 1e-9
+            near_pos = min(abs(o["ap_new"][i]), abs(o["as_new"][i])) < 1e-9 * (abs(o["delta_p"][i]) + abs(o["delta_s"][i]))
+            assert near_metropolis or near_pos, f"walker {w}: unflagged decision mismatch at move {i}"
+            flagged += 1
+            end = i                      # chains diverge after a flipped decision: stop comparing this walker
+            assert stop_on_flagged
+        sl = slice(0, end)
+        assert _ulp_close(g["rho"][sl], o["rho"][sl]).all()
+        assert _ulp_close(g["delta_p"][sl], o["delta_p"][sl]).all()
+        assert _ulp_close(g["delta_s"][sl], o["delta_s"][sl]).all()
+        # acceptance threshold: thr = -T ln u
+        np.testing.assert_allclose(g["thr"][sl], -Tm[sl] * o["ln_u"][sl], rtol=1e-14)
+        ev = (g["flags"][sl] & 4) != 0
+        assert (ev | ((g["flags"][sl] & 1) == 0)).all()            # every feasible move was evaluated
+        err = np.abs(g["dchi2"][sl] - o["dchi2"][sl])[ev]
+        tol = 1e-12 * o["l1"][sl][ev]
+        assert (err <= tol).all(), f"walker {w}: dchi2 off by up to {np.max(err / o['l1'][sl][ev]):.3e} of l1"
+        for fld, dl in (("ap_new", "delta_p"), ("as_new", "delta_s")):
+            scale = np.abs(o[dl][sl]) + np.abs(o[fld][sl])
+            assert (np.abs(g[fld][sl] - o[fld][sl]) <= 1e-12 * scale + 1e-300).all()
+    return flagged
+
+
+# ------------------------------------------------------------------------------------------------
+def test_init_forward_and_residue_match_oracle():
+    """A1: exponential-tilt start (G4), M = a K (Eq. 7), chi^2 (Eq. 9)."""
+    w = wl.make("tiny", simpson_intervals=100_000)
+    s = _sail(w, 64)
+    s.init_walkers(64, w.A, w.B, SEED)
+    o = _oracle(w, 64)
+    a, c2 = s.get()
+    np.testing.assert_allclose(a, o.a, rtol=1e-12)
+    np.testing.assert_allclose(s.get_model(), o.M, rtol=1e-13)
+    np.testing.assert_allclose(c2, o.chi2, rtol=1e-8)
+    acc, ev, y = s.stats()
+    assert (acc == 0).all() and (ev == 0).all() and (y == 1.0).all()
+    s.close()
+
+
+@pytest.mark.parametrize("lanes", [32, 16, 8])
+def test_tiny_full_anneal_trace_and_sequence_parity(lanes):
+    """configs[0] in full: 64 walkers x 2000 sweeps x 64 moves, every move traced (L1, L2, L3)."""
+    w = wl.make("tiny", simpson_intervals=100_000)
+    o = _oracle(w, w.W)
+    s = _sail(w, w.W)
+    s.init_walkers(w.W, w.A, w.B, SEED, spectra=o.a)          # identical start on both sides
+    flagged = 0
+    chunk = 250
+    for c0 in range(0, w.n_sweeps, chunk):
+        T = w.schedule[c0:c0 + chunk]
+        tg, fg = s.anneal(T, w.eta, lanes_per_walker=lanes, trace_walkers=(0, w.W), want_flags=True)
+        to, fo = o.anneal(T, trace_walkers=(0, w.W), want_flags=True)
+        flagged += compare_traces(tg, to, T)
+        if flagged == 0:
+            assert ((fg & 3) == fo).all()
+            assert ((tg["flags"] & 3) == fg).all()
+    assert flagged <= 1                                        # expected ~0 (P ~ 1e-2 per whole run)
+    if flagged == 0:
+        a, c2 = s.get()
+        np.testing.assert_allclose(a, o.a, rtol=0, atol=1e-9 * o.a.max())
+        np.testing.assert_allclose(c2, o.chi2, rtol=1e-9)
+        np.testing.assert_allclose(a.mean(axis=0), o.a.mean(axis=0), rtol=0, atol=1e-9 * o.a.mean(axis=0).max())
+        acc, ev, y = s.stats()
+        assert (acc == o.acc).all() and (ev == o.feas).all()
+        np.testing.assert_allclose(y, o.y, rtol=1e-15)
+        wm = w.omega + 0.5 * w.domega
+        np.testing.assert_allclose(a.sum(axis=1), w.A, rtol=1e-11)     # sum rules survive the whole anneal
+        np.testing.assert_allclose((a * wm).sum(axis=1), w.B, rtol=1e-11)
+        assert (a >= 0).all()
+    s.close()
+
+
+@pytest.mark.parametrize("name,W,lanes,n_sw", [("small", 97, 32, 12), ("small", 97, 16, 12), ("small", 50, 8, 8),
+                                               ("branching", 70, 16, 4), ("branching", 33, 32, 4),
+                                               ("noise", 40, 32, 3), ("noise", 40, 16, 3), ("stress", 35, 32, 2)])
+def test_ragged_sizes_trace_parity(name, W, lanes, n_sw):
+    """Other configs' grids (N_tau = 100, 200, 256, 512: several tau-points per lane with a ragged tail,
+    factored start tables for the large N_omega) at walker counts that do not fill the last warp."""
+    w = wl.make(name, simpson_intervals=20_000)
+    o = _oracle(w, W)
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED)
+    np.testing.assert_allclose(s.get()[0], o.a, rtol=1e-12)
+    s.set_walkers(0, o.a)
+    T = wl.geometric_schedule(1.0, 0.5, n_sw)
+    tg, fg = s.anneal(T, w.eta, lanes_per_walker=lanes, trace_walkers=(0, W), want_flags=True)
+    to, fo = o.anneal(T, trace_walkers=(0, W), want_flags=True)
+    assert compare_traces(tg, to, T) == 0
+    assert ((fg & 3) == fo).all()
+    a, c2 = s.get()
+    np.testing.assert_allclose(a, o.a, rtol=0, atol=1e-10 * o.a.max())
+    np.testing.assert_allclose(c2, o.chi2, rtol=1e-9)
+    np.testing.assert_allclose(s.get_model(), o.M, rtol=1e-10)
+    s.close()
+
+
+def test_split_calls_do_not_change_the_stream_and_resync_matches_oracle():
+    """Absolute sweep counter (one 6-sweep call == 2 + 4); A7: resync = forward(a) + residue."""
+    w = wl.make("small", simpson_intervals=20_000)
+    W = 64
+    T = wl.geometric_schedule(1.0, 0.2, 6)
+    s1 = _sail(w, W); s1.init_walkers(W, w.A, w.B, SEED); s1.anneal(T, w.eta)
+    s2 = _sail(w, W); s2.init_walkers(W, w.A, w.B, SEED); s2.anneal(T[:2], w.eta); s2.anneal(T[2:], w.eta)
+    a1, c1 = s1.get(); a2, c2 = s2.get()
+    np.testing.assert_array_equal(a1, a2)
+    np.testing.assert_array_equal(c1, c2)
+    s1.resync()
+    K = oracle.kernel_table(w.omega, w.tau)
+    M = s1.get_model()
+    _, c1r = s1.get(spectra=False)
+    for i in range(0, W, 7):
+        Mo = oracle.forward(K, a1[i])
+        np.testing.assert_allclose(M[i], Mo, rtol=1e-13)
+        assert c1r[i] == pytest.approx(oracle.chi2(Mo, w.F, w.sigma), rel=1e-8)
+    np.testing.assert_allclose(c1r, c1, rtol=1e-8)             # incremental chi^2 had not drifted
+    # resync_every inside sail_anneal: same chain, chi^2 refreshed at the boundary
+    s3 = _sail(w, W); s3.init_walkers(W, w.A, w.B, SEED); s3.anneal(T, w.eta, resync_every=3)
+    o = _oracle(w, W); o.anneal(T, resync_every=3)
+    a3, c3 = s3.get()
+    np.testing.assert_allclose(a3, o.a, rtol=0, atol=1e-10 * o.a.max())
+    np.testing.assert_allclose(c3, o.chi2, rtol=1e-9)
+    for s in (s1, s2, s3):
+        s.close()
+
+
+@pytest.mark.parametrize("W,t", [(64, 0.1), (3000, 0.1), (3000, 1.0), (1025, 0.0)])
+def test_branching_parity(W, t):
+    """A8: multipliers, donor map and imprinted state against the oracle from the same (a, chi^2)."""
+    w = wl.make("tiny", simpson_intervals=20_000)
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED)
+    s.anneal(np.full(3, 1.0), w.eta)
+    a0, c0 = s.get()
+    o = _oracle(w, W, spectra=a0)
+    o.chi2[:] = c0                                   # identical weights input on both sides
+    o.sweep = 3
+    T = float(np.std(c0)) if t > 0 else float(np.std(c0)) * 0.3
+    info, mult, donor = s.branch(T, t, want_maps=True)
+    n_rec, mo, do = o.branch(T, t)
+    assert mult.sum() == W
+    assert (mult == mo).all()
+    assert (donor == do).all()
+    assert info.n_recipients == n_rec == (mult == 0).sum()
+    assert info.max_multiplier == mult.max()
+    assert info.chi2_min == c0.min()
+    a1, c1 = s.get()
+    np.testing.assert_array_equal(a1, o.a)           # same two roundings per element on both sides
+    rec = donor >= 0
+    np.testing.assert_allclose(c1[rec], o.chi2[rec], rtol=1e-8)
+    np.testing.assert_array_equal(c1[~rec], c0[~rec])
+    np.testing.assert_allclose(s.get_model()[rec], o.M[rec], rtol=1e-12)
+    if t == 1.0:
+        np.testing.assert_array_equal(a1[rec], a0[donor[rec]])
+    if t == 0.0:
+        np.testing.assert_array_equal(a1, a0)
+    s.close()
+
+
+def test_branch_then_anneal_protocol_lockstep():
+    """Reduced-W run of the Branching protocol (blocks of sweeps + branching), state re-injected from the
+    GPU into the oracle at every block so that both sides start each block from identical inputs."""
+    w = wl.make("branching", simpson_intervals=20_000)
+    W, blk = 256, 3
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED)
+    o = _oracle(w, W)
+    sched = wl.geometric_schedule(1.0, 0.3, 4 * blk)
+    for b in range(4):
+        a_g, c_g = s.get()
+        _, _, y_g = s.stats()
+        o.a[:] = a_g; o.resync(); o.y[:] = y_g
+        np.testing.assert_allclose(o.chi2, c_g, rtol=1e-8)
+        T = sched[b * blk:(b + 1) * blk]
+        tg, _ = s.anneal(T, w.eta, trace_walkers=(100, 140))
+        to, _ = o.anneal(T, trace_walkers=(100, 140))
+        assert compare_traces(tg, to, T) == 0
+        a_g, c_g = s.get()
+        np.testing.assert_allclose(a_g, o.a, rtol=0, atol=1e-10 * o.a.max())
+        o.a[:] = a_g; o.chi2[:] = c_g
+        info, mult, donor = s.branch(float(T[-1]) * float(np.std(c_g)), w.t_imprint, want_maps=True)
+        n_rec, mo, do = o.branch(float(T[-1]) * float(np.std(c_g)), w.t_imprint)
+        assert (mult == mo).all() and (donor == do).all()
+        np.testing.assert_array_equal(s.get()[0], o.a)
+    s.close()
+
+
+def test_bench_configuration_sampled_parity():
+    """configs[1] (Small) at FULL size in the launch configuration bench.py times (auto lanes, W = 4096):
+    walkers [2000, 2064) are traced on the GPU for whole sweeps at several points of the anneal and the oracle
+    replays those sweeps from the injected GPU state."""
+    w = wl.make("small", simpson_intervals=100_000)
+    s = _sail(w, w.W)
+    s.init_walkers(w.W, w.A, w.B, SEED)
+    lo, hi = 2000, 2064
+    done = 0
+    for upto in (0, 40, 400):
+        if upto > done:
+            s.anneal(w.schedule[done:upto], w.eta)
+            done = upto
+        a_g, c_g = s.get()
+        _, _, y_g = s.stats()
+        o = _oracle(w, hi - lo, spectra=a_g[lo:hi])
+        np.testing.assert_allclose(o.chi2, c_g[lo:hi], rtol=1e-7)
+        o.y[:] = y_g[lo:hi]
+        o.sweep = done
+        # the oracle's walker index is the Philox counter: replay with absolute indices
+        tr_o = np.zeros((hi - lo, 2, w.n_omega), dtype=oracle.TRACE_DTYPE)
+        T = w.schedule[done:done + 2]
+        tg, _ = s.anneal(T, w.eta, trace_walkers=(lo, hi))
+        for i in range(hi - lo):
+            for k in range(2):
+                for m in range(w.n_omega):
+                    rec = _oracle_move(o, i, lo + i, done + k, m, T[k])
+                    tr_o[i, k, m] = rec
+                _end_sweep(o, i, tr_o[i, k])
+        done += 2
+        assert compare_traces(tg, tr_o, T) == 0
+        a2, c2 = s.get()
+        np.testing.assert_allclose(a2[lo:hi], o.a, rtol=0, atol=1e-10 * o.a.max())
+        np.testing.assert_allclose(c2[lo:hi], o.chi2, rtol=1e-9)
+    s.close()
+
+
+def _oracle_move(o, local, walker_id, sweep, move, T):
+    """orc_move with an explicit Philox walker id (the oracle object holds only the sampled walkers)."""
+    import ctypes as C
+    tr = np.zeros(1, dtype=oracle.TRACE_DTYPE)
+    c2 = C.c_double(o.chi2[local])
+    oracle.lib().orc_move(C.byref(o.P), C.c_int64(walker_id), C.c_int64(sweep), C.c_int32(move), C.c_double(T),
+                          C.c_double(float(o.y[local])), o.a[local].ctypes.data_as(C.c_void_p),
+                          o.M[local].ctypes.data_as(C.c_void_p), C.byref(c2), tr.ctypes.data_as(C.c_void_p))
+    o.chi2[local] = c2.value
+    return tr[0]
+
+
+def _end_sweep(o, local, sweep_trace):
+    rate = ((sweep_trace["flags"] & 2) != 0).sum() / sweep_trace.size
+    o.y[local] = oracle.amp_factor(rate)
+
+
+def test_errors_and_limits_on_device():
+    from paper_1609_07936_b200.binding import Sail, SailError, SAIL_ERR_ARG, SAIL_ERR_STATE, SAIL_ERR_GRID
+    w = wl.make("tiny", simpson_intervals=20_000)
+    s = _sail(w, 8)
+    with pytest.raises(SailError) as e:
+        s.anneal(np.ones(2), w.eta)
+    assert e.value.code == SAIL_ERR_STATE
+    with pytest.raises(SailError) as e:
+        s.init_walkers(9, w.A, w.B, SEED)
+    assert e.value.code == SAIL_ERR_ARG
+    with pytest.raises(SailError):
+        s.init_walkers(8, w.A, w.A * 100.0, SEED)              # B/A outside the grid
+    s.init_walkers(8, w.A, w.B, SEED)
+    for bad in (dict(eta=0.0), dict(eta=1.5)):
+        with pytest.raises(SailError):
+            s.anneal(np.ones(2), **bad)
+    with pytest.raises(SailError):
+        s.anneal(np.array([1.0, -1.0]), w.eta)
+    s.anneal(np.ones(0), w.eta)                                  # empty schedule is a no-op
+    a, _ = s.get()
+    np.testing.assert_allclose(a.sum(axis=1), w.A, rtol=1e-13)
+    om = w.omega.copy(); om[3] += 1e-3
+    with pytest.raises(SailError) as e:
+        Sail(om, w.tau, w.F, w.sigma, max_walkers=8)
+    assert e.value.code == SAIL_ERR_GRID
+    # library-owned workspace path + sigma = None (the paper's unweighted Eq. 9)
+    s2 = Sail(w.omega, w.tau, w.F, None, max_walkers=4, torch_workspace=False)
+    s2.init_walkers(4, w.A, w.B, SEED)
+    _, c2 = s2.get()
+    o = oracle.Oracle(w.omega, w.tau, w.F, None, w.A, w.B, w.eta, SEED); o.init_walkers(4)
+    np.testing.assert_allclose(c2, o.chi2, rtol=1e-8)
+    assert s2.launch_count() > 0
+    s.close(); s2.close()
+
+
+def test_single_tau_and_single_walker_degenerate_cases():
+    """N_tau = 1 (only tau = 0: Eq. 16 makes every move chi^2-neutral) and W = 1."""
+    omega = np.arange(8) * 0.5
+    tau = np.array([0.0])
+    A, B = 4.0, 4.0 * 1.6
+    F = np.array([A * 0.5 / (2 * np.pi)])
+    from paper_1609_07936_b200.binding import Sail
+    s = Sail(omega, tau, F, np.array([1e-3]), max_walkers=1)
+    s.init_walkers(1, A, B, 7)
+    o = oracle.Oracle(omega, tau, F, np.array([1e-3]), A, B, 0.3, 7); o.init_walkers(1)
+    T = np.full(5, 1.0)
+    tg, fg = s.anneal(T, 0.3, trace_walkers=(0, 1), want_flags=True)
+    to, fo = o.anneal(T, trace_walkers=(0, 1), want_flags=True)
+    assert ((fg & 3) == fo).all()
+    a, _ = s.get()
+    np.testing.assert_allclose(a, o.a, rtol=0, atol=1e-12)
+    s.close()
