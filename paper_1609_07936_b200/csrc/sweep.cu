@@ -77,15 +77,14 @@ __global__ void __launch_bounds__(MAXW * 32, 1) sweep_kernel(const SweepArgs P)
         double *a_w = P.a + (size_t)w * n_omega;
 
         // ---- load the walker's residual state into registers --------------------------------------
-        double mt[C], G2[C], Wt[C], d[C];
+        double mt[C], G2[C], Wt[C], d[C], fv[C];
 #pragma unroll
         for (int i = 0; i < C; ++i) {
             const int j = sub + G * i;
             const bool ok = j < P.n_tau;
             mt[i] = ok ? P.mt[(size_t)w * P.n_tau + j] : 0.0;
             Wt[i] = ok ? P.Wj[j] : 0.0;
-            const double f = ok ? P.fj[j] : 0.0;
-            G2[i] = 2.0 * Wt[i] * (mt[i] - f);
+            fv[i] = ok ? P.fj[j] : 0.0;
             d[i] = 0.0;
         }
         double chi2 = P.chi2[w];
@@ -98,6 +97,10 @@ __global__ void __launch_bounds__(MAXW * 32, 1) sweep_kernel(const SweepArgs P)
             const long long sweep = P.sweep0 + isw;
             const double T = P.T[isw];
             int acc_sweep = 0;
+            // G2 is a pure function of mt at every sweep start, so splitting a run into several calls
+            // (state round-trips through global memory) reproduces the single-call chain bit for bit
+#pragma unroll
+            for (int i = 0; i < C; ++i) G2[i] = 2.0 * Wt[i] * (mt[i] - fv[i]);
 
             for (int m0 = 0; m0 < n_omega; m0 += G) {
                 const int nb = min(G, n_omega - m0);
