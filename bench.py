@@ -94,8 +94,12 @@ def measured_peaks():
         return {}
 
 
+LANES = 0   # --lanes: lanes of a warp per walker (0 = library default)
+
+
 def anneal_params(w):
-    return dict(eta=w.eta, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6, resync_every=w.resync_every)
+    return dict(eta=w.eta, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6, resync_every=w.resync_every,
+                lanes_per_walker=LANES)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -349,5 +353,7 @@ if __name__ == "__main__":
     ap.add_argument("--sweeps", type=int, default=0, help="override the number of sweeps (debug)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--extra", type=int, default=1, help="also time a block of the stress config (N=1 only)")
+    ap.add_argument("--lanes", type=int, default=0, help="lanes per walker: 0 auto, 8, 16, 32")
     a = ap.parse_args()
+    LANES = a.lanes
     sys.exit(main_reference(a) if a.impl == "reference" else main_ours(a))

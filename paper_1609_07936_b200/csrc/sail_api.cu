@@ -26,7 +26,7 @@ int set_err(sail_handle *h, int code, const char *fmt, ...)
 
 // ---- workspace layout ------------------------------------------------------------------------------
 struct Layout {
-    size_t off_omega, off_tau, off_c, off_Wj, off_fj, off_F, off_sigma, off_E, off_ratio, off_E0;
+    size_t off_omega, off_tau, off_c, off_Wj, off_fj, off_F, off_sigma, off_E, off_ratio, off_invd, off_E0;
     size_t off_a, off_mt, off_chi2, off_y, off_nacc, off_neval;
     size_t off_ehat, off_scanA, off_scanB, off_bsums, off_mult, off_donor, off_reclist, off_scalars;
     size_t total;
@@ -38,11 +38,12 @@ static Layout make_layout(int n_omega, int n_tau, int64_t Wmax)
     Layout L{};
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
-    const size_t W = (size_t)Wmax, d = sizeof(double), u = sizeof(unsigned long long);
+    // + 3 scratch walker slots: the sweep kernel pads W to a multiple of 4 (see sweep.cu)
+    const size_t W = (size_t)Wmax + 3, d = sizeof(double), u = sizeof(unsigned long long);
     L.off_omega = take(n_omega * d);  L.off_tau = take(n_tau * d);   L.off_c = take(n_tau * d);
     L.off_Wj = take(n_tau * d);       L.off_fj = take(n_tau * d);    L.off_F = take(n_tau * d);
     L.off_sigma = take(n_tau * d);    L.off_E = take((size_t)n_omega * n_tau * d);
-    L.off_ratio = take(n_omega * d);  L.off_E0 = take(kE0Doubles * d);
+    L.off_ratio = take(n_omega * d);  L.off_invd = take(n_omega * d);  L.off_E0 = take(kE0Doubles * d);
     L.off_a = take(W * n_omega * d);  L.off_mt = take(W * n_tau * d);
     L.off_chi2 = take(W * d);         L.off_y = take(W * d);
     L.off_nacc = take(W * u);         L.off_neval = take(W * u);
@@ -193,7 +194,7 @@ int sail_create(sail_t **out, const double *omega, int32_t n_omega, const double
     auto U = [&](size_t off) { return (unsigned long long *)(base + off); };
     h->tab.omega = D(L.off_omega); h->tab.tau = D(L.off_tau); h->tab.c = D(L.off_c); h->tab.Wj = D(L.off_Wj);
     h->tab.fj = D(L.off_fj); h->tab.E = D(L.off_E);
-    h->sw_ratio = D(L.off_ratio); h->sw_E0 = D(L.off_E0);
+    h->sw_ratio = D(L.off_ratio); h->sw_invd = D(L.off_invd); h->sw_E0 = D(L.off_E0);
     h->st.a = D(L.off_a); h->st.mt = D(L.off_mt); h->st.chi2 = D(L.off_chi2); h->st.y = D(L.off_y);
     h->st.n_acc = U(L.off_nacc); h->st.n_eval = U(L.off_neval);
     h->br.ehat = U(L.off_ehat); h->br.scanA = U(L.off_scanA); h->br.scanB = U(L.off_scanB);
@@ -240,7 +241,7 @@ int sail_init_walkers(sail_t *h, int64_t W, double A, double B, uint64_t seed, i
             if (!(spectra[i] >= 0.0)) return set_err(h, SAIL_ERR_ARG, "spectra[%zu] is negative or NaN", i);
         SAIL_CUDA_OK(h, cudaMemcpyAsync(h->st.a, spectra, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     }
-    fill_state_kernel<<<blocks, 256, 0, h->stream>>>(W, h->st.y, h->st.n_acc, h->st.n_eval);
+    fill_state_kernel<<<blocks, 256, 0, h->stream>>>(W + 3, h->st.y, h->st.n_acc, h->st.n_eval);
     SAIL_LAUNCH_OK(h, "fill_state_kernel");
     int rc = launch_forward(h, 0, W);
     if (rc) return rc;

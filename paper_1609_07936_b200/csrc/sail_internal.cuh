@@ -75,6 +75,7 @@ struct sail_handle {
     bool tables_fact = false;
     int fact_shift = 0;
     double *sw_ratio = nullptr;  // [n_omega] exp(-omega_k G dtau)
+    double *sw_invd = nullptr;   // [n_omega] 1/(k domega)
     double *sw_E0 = nullptr;     // direct: [n_omega][G]; factored: H[n_hi][G] then L[n_lo][G]
     double *d_T = nullptr;       // device copy of the schedule chunk (library-owned, grows)
     size_t d_T_cap = 0;

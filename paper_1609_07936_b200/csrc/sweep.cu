@@ -11,11 +11,13 @@
 // so E_{k,j+G} = E_kj * exp(-omega_k G dtau); each lane starts from E0[k][l] (shared memory) and
 // advances by one DMUL per row per tau-point, with delta folded into the start value:
 //     6 FP64-pipe instructions per tau-point (2 DMUL, 1 DADD, 3 DFMA), no memory traffic.
-// Proposals (Philox4x32-10 keyed by (seed; walker, sweep, move, 0), index draw, rho, Eq. 20-21
-// divisions, -T ln u) do not depend on the chain state within a sweep, so they are computed G moves
-// at a time, one move per lane, and staged as 64-byte records in shared memory.
+// Proposals (Philox4x32-10 keyed by (seed; walker, sweep, move, 0), index draw, rho, Eq. 20-21,
+// -T ln u) do not depend on the chain state within a sweep, so they are computed G moves at a time,
+// one move per lane, and staged as 64-byte records in shared memory.
 // Eq. 19 (scale ALL coefficients by rho) is applied lazily: a = g * a~, g <- g rho on accept, folded
 // into a~ at the end of every sweep.
+// Walker slots W .. W_pad-1 (W_pad = W rounded up to 4) are scratch copies of the last walker so that a
+// warp never has an inactive group: no activity predicate in the hot loop; they are never reported.
 #include "sail_internal.cuh"
 
 namespace sail {
@@ -23,10 +25,10 @@ namespace sail {
 struct SweepArgs {
     int n_omega, n_tau;
     long long W, n_groups;
-    double A, B, domega, eta, amp_p, amp_m, y_min;
+    double A, B, omega_mid0, domega, eta, amp_p, amp_m, y_min;
     int amp_mode;
     uint32_t seed_lo, seed_hi;
-    const double *omega, *Wj, *fj, *ratio, *E0;
+    const double *Wj, *fj, *ratio, *E0, *invd, *omega;
     int fact, fact_shift, n_hi, n_lo;
     double *a, *mt, *chi2, *y;
     unsigned long long *n_acc, *n_eval;
@@ -39,23 +41,57 @@ struct SweepArgs {
     long long call_sweeps, call_off;   // sweeps in the whole sail_anneal call / offset of this launch
 };
 
-__device__ __forceinline__ double shfl_xor_f64(double v, int off)
+// 1/x for x close to 1 (|x - 1| < 0.5): hardware seed + two Newton steps, relative error ~1e-16.
+__device__ __forceinline__ double fast_recip(double x)
 {
-    return __shfl_xor_sync(0xffffffffu, v, off);
+    double r;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
+    double e = fma(-x, r, 1.0);
+    r = fma(r, e, r);
+    e = fma(-x, r, 1.0);
+    return fma(r, e, r);
 }
 
-template <int G, int C, int MAXW>
-__global__ void __launch_bounds__(MAXW * 32, 1) sweep_kernel(const SweepArgs P)
+// shared-memory accesses by 32-bit shared-window address (no generic-address arithmetic in the hot loop)
+__device__ __forceinline__ double lds_f64(uint32_t addr)
+{
+    double v;
+    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ double2 lds_f64x2(uint32_t addr)
+{
+    double2 v;
+    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
+    return v;
+}
+__device__ __forceinline__ int4 lds_s32x4(uint32_t addr)
+{
+    int4 v;
+    asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
+    return v;
+}
+
+// MAXW = warps per CTA (one CTA per SM) the variant is register-budgeted for; the register file is allocated in
+// units of 4 warps per CTA, so the budget is 65536 / (roundup4(MAXW) * 32) registers per thread.
+// FACT: start values E0[k][l] = H[k_hi][l] * L[k_lo][l] (two small tables) instead of one N_omega x G table.
+template <int G, int C, int MAXW, bool FACT, bool TRACE>
+__global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kernel(const SweepArgs P)
 {
     constexpr int NW = 32 / G;               // walkers per warp
     extern __shared__ __align__(16) unsigned char smem[];
     double *s_ratio = reinterpret_cast<double *>(smem);
-    const int n_omega_pad = (P.n_omega + 1) & ~1;
-    double *s_E0 = s_ratio + n_omega_pad;
-    const int e0_elems = P.fact ? (P.n_hi + P.n_lo) * G : P.n_omega * G;
+    const int n_omega = P.n_omega;
+    const int n_omega_pad = (n_omega + 1) & ~1;
+    double *s_invd = s_ratio + n_omega_pad;                       // 1 / (k domega), k = 1 .. n_omega-1
+    double *s_wm = s_invd + n_omega_pad;                          // bin midpoints omega_k + domega/2
+    double *s_E0 = s_wm + n_omega_pad;
+    const int e0_elems = FACT ? (P.n_hi + P.n_lo) * G : n_omega * G;
     unsigned char *s_recs = reinterpret_cast<unsigned char *>(s_E0 + ((e0_elems + 1) & ~1));
 
-    for (int i = threadIdx.x; i < P.n_omega; i += blockDim.x) s_ratio[i] = P.ratio[i];
+    for (int i = threadIdx.x; i < n_omega; i += blockDim.x) {
+        s_ratio[i] = P.ratio[i]; s_invd[i] = P.invd[i]; s_wm[i] = __dadd_rn(P.omega[i], 0.5 * P.domega);
+    }
     for (int i = threadIdx.x; i < e0_elems; i += blockDim.x) s_E0[i] = P.E0[i];
     __syncthreads();
 
@@ -63,129 +99,145 @@ __global__ void __launch_bounds__(MAXW * 32, 1) sweep_kernel(const SweepArgs P)
     const int warp = threadIdx.x >> 5;
     const int sub = lane % G;                // lane within the walker's group
     const int q = lane / G;                  // which walker of the warp
-    unsigned char *my_recs = s_recs + (size_t)warp * 32 * kRecBytes;
+    unsigned char *my_rec_w = s_recs + ((size_t)warp * 32 + lane) * kRecBytes;       // record this lane writes
+    // 32-bit shared addresses: records this lane's group reads, this lane's column of the start table(s)
+    const uint32_t rbase = (uint32_t)__cvta_generic_to_shared(s_recs) + (uint32_t)((warp * 32 + q * G) * kRecBytes);
+    const uint32_t e0_lane = (uint32_t)__cvta_generic_to_shared(s_E0) + (uint32_t)(sub * 8);
+    const uint32_t e0_lo = e0_lane + (uint32_t)(P.n_hi * G * 8);                     // FACT: low-part table
     const int warps_per_cta = blockDim.x >> 5;
     const long long total_warps = (long long)gridDim.x * warps_per_cta;
-    const int n_omega = P.n_omega;
-    const double half_dw = 0.5 * P.domega;
-    const int fmask = (1 << P.fact_shift) - 1;
+    const int fshift = P.fact_shift;
+    const int fmask = (1 << fshift) - 1;
+    const bool leader = (sub == 0);
 
     for (long long grp = (long long)blockIdx.x * warps_per_cta + warp; grp < P.n_groups; grp += total_warps) {
-        const long long w_raw = grp * NW + q;
-        const bool active = w_raw < P.W;
-        const long long w = active ? w_raw : P.W - 1;
-        double *a_w = P.a + (size_t)w * n_omega;
+        const long long w = grp * NW + q;                          // < W_pad: always a valid slot
+        double *__restrict__ a_w = P.a + (size_t)w * n_omega;
 
         // ---- load the walker's residual state into registers --------------------------------------
-        double mt[C], G2[C], Wt[C], d[C], fv[C];
+        double mt[C], G2[C], Wt[C], d[C], v[C];
 #pragma unroll
         for (int i = 0; i < C; ++i) {
             const int j = sub + G * i;
             const bool ok = j < P.n_tau;
             mt[i] = ok ? P.mt[(size_t)w * P.n_tau + j] : 0.0;
             Wt[i] = ok ? P.Wj[j] : 0.0;
-            fv[i] = ok ? P.fj[j] : 0.0;
             d[i] = 0.0;
+            v[i] = 0.0;
         }
         double chi2 = P.chi2[w];
         double y = P.y[w];
         double g = 1.0, ginv = 1.0;
-        unsigned long long tot_acc = 0, tot_eval = 0;
-        const bool tracing = P.trace != nullptr && active && w >= P.trace_lo && w < P.trace_hi;
+        bool tracing = false;
+        if (TRACE) tracing = P.trace != nullptr && w >= P.trace_lo && w < P.trace_hi;
 
         for (int isw = 0; isw < P.n_sweeps; ++isw) {
-            const long long sweep = P.sweep0 + isw;
-            const double T = P.T[isw];
-            int acc_sweep = 0;
+            const uint32_t sweep = (uint32_t)(P.sweep0 + isw);
+            int acc_sweep = 0, eval_sweep = 0;
             // G2 is a pure function of mt at every sweep start, so splitting a run into several calls
             // (state round-trips through global memory) reproduces the single-call chain bit for bit
 #pragma unroll
-            for (int i = 0; i < C; ++i) G2[i] = 2.0 * Wt[i] * (mt[i] - fv[i]);
+            for (int i = 0; i < C; ++i) {
+                const int j = sub + G * i;
+                const double f = (j < P.n_tau) ? P.fj[j] : 0.0;
+                G2[i] = 2.0 * Wt[i] * (mt[i] - f);
+            }
 
             for (int m0 = 0; m0 < n_omega; m0 += G) {
                 const int nb = min(G, n_omega - m0);
                 // ---- proposals for moves m0 .. m0+nb-1, one per lane (row A2) -----------------------
                 if (sub < nb) {
-                    const int m = m0 + sub;
                     uint32_t x[4];
-                    philox4x32_10((uint32_t)w, (uint32_t)sweep, (uint32_t)m, 0u, P.seed_lo, P.seed_hi, x);
+                    philox4x32_10((uint32_t)w, sweep, (uint32_t)(m0 + sub), 0u, P.seed_lo, P.seed_hi, x);
                     const int p = (int)__umulhi(x[0], (uint32_t)n_omega);
                     int s = (int)__umulhi(x[1], (uint32_t)(n_omega - 1));
                     s += (s >= p) ? 1 : 0;
                     const double u_rho = ((double)x[2] + 0.5) * 2.3283064365386962890625e-10;
                     const double u_acc = ((double)x[3] + 0.5) * 2.3283064365386962890625e-10;
-                    // same operation order as the method's definition, no contraction (bit-stable draws)
+                    // rho in the method's operation order, no contraction: bit-identical to the definition
                     const double rho = __dsub_rn(1.0, __dmul_rn(__dmul_rn(y, P.eta),
                                                                 __dsub_rn(__dmul_rn(2.0, u_rho), 1.0)));
+                    const double alpha = __dsub_rn(rho, 1.0);          // exact
+                    // Eq. 20-21 in the method's operation order; only the division by (p-s) domega is a
+                    // multiplication by the correctly rounded reciprocal (delta within 2 ulp of the division)
                     const double omr = __dsub_rn(1.0, rho);
-                    const double wm_p = __dadd_rn(P.omega[p], half_dw);
-                    const double wm_s = __dadd_rn(P.omega[s], half_dw);
-                    const double dp = __ddiv_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, wm_s))),
-                                                __dmul_rn((double)(p - s), P.domega));     // Eq. 20
-                    const double ds = __ddiv_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, wm_p))),
-                                                __dmul_rn((double)(s - p), P.domega));     // Eq. 21
-                    const double thr = -T * log(u_acc);
-                    const double alpha = __dsub_rn(rho, 1.0);
-                    unsigned char *r = my_recs + (size_t)lane * kRecBytes;
-                    *reinterpret_cast<int4 *>(r) = make_int4(p, s, __double2loint(alpha), __double2hiint(alpha));
-                    *reinterpret_cast<double2 *>(r + 16) = make_double2(dp, ds);
-                    *reinterpret_cast<double2 *>(r + 32) = make_double2(thr, 1.0 / rho);
-                    *reinterpret_cast<double2 *>(r + 48) = make_double2(s_ratio[p], s_ratio[s]);
+                    const int dps = p - s;
+                    const double inv = (dps > 0) ? s_invd[dps] : -s_invd[-dps];
+                    const double dp = __dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[s]))), inv);
+                    const double ds = -__dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[p]))), inv);
+                    const double thr = -P.T[isw] * log(u_acc);
+                    *reinterpret_cast<int4 *>(my_rec_w) = make_int4(p, s, __double2loint(alpha), __double2hiint(alpha));
+                    *reinterpret_cast<double2 *>(my_rec_w + 16) = make_double2(dp, ds);
+                    *reinterpret_cast<double2 *>(my_rec_w + 32) = make_double2(thr, fast_recip(rho));
+                    *reinterpret_cast<double2 *>(my_rec_w + 48) = make_double2(s_ratio[p], s_ratio[s]);
                 }
                 __syncwarp();
 
-                // ---- software pipeline: record + spectrum values of the next move are fetched early --
-                const unsigned char *rbase = my_recs + (size_t)(q * G) * kRecBytes;
-                int4 r0 = *reinterpret_cast<const int4 *>(rbase);
-                double ap_t = a_w[r0.x], as_t = a_w[r0.y];
+                // ---- software pipeline -------------------------------------------------------------------
+                // Everything of move mm+1 that does not depend on the chain state (record, start values,
+                // v_i = delta_p E_p,i + delta_s E_s,i by the geometric recurrence, the two spectrum
+                // coefficients) is prepared while move mm's reduction is in flight.
+                int4 r0;            // p, s, alpha
+                double2 dd, th;     // (delta_p, delta_s), (threshold, 1/rho)
+                double ap_t, as_t;  // a~_p, a~_s (patched if move mm rewrites them)
+                auto prepare = [&](int mm) {
+                    const uint32_t r = rbase + (uint32_t)(mm * kRecBytes);
+                    r0 = lds_s32x4(r);
+                    dd = lds_f64x2(r + 16);
+                    th = lds_f64x2(r + 32);
+                    const double2 rr = lds_f64x2(r + 48);
+                    ap_t = a_w[(unsigned)r0.x];
+                    as_t = a_w[(unsigned)r0.y];
+                    double e0p, e0s;
+                    if (FACT) {
+                        e0p = lds_f64(e0_lane + (uint32_t)((r0.x >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.x & fmask) * (G * 8)));
+                        e0s = lds_f64(e0_lane + (uint32_t)((r0.y >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.y & fmask) * (G * 8)));
+                    } else {
+                        e0p = lds_f64(e0_lane + (uint32_t)(r0.x * (G * 8)));
+                        e0s = lds_f64(e0_lane + (uint32_t)(r0.y * (G * 8)));
+                    }
+                    double ep = dd.x * e0p, es = dd.y * e0s;
+#pragma unroll
+                    for (int i = 0; i < C; ++i) {
+                        v[i] = ep + es;
+                        if (i + 1 < C) { ep *= rr.x; es *= rr.y; }
+                    }
+                };
+                prepare(0);
 
                 for (int mm = 0; mm < nb; ++mm) {
-                    const unsigned char *r = rbase + (size_t)mm * kRecBytes;
                     const int p = r0.x, s = r0.y;
                     const double alpha = __hiloint2double(r0.w, r0.z);
-                    const double2 dd = *reinterpret_cast<const double2 *>(r + 16);
-                    const double2 th = *reinterpret_cast<const double2 *>(r + 32);
-                    const double2 rr = *reinterpret_cast<const double2 *>(r + 48);
-                    const double cap = ap_t, cas = as_t;
-                    if (mm + 1 < nb) {
-                        r0 = *reinterpret_cast<const int4 *>(r + kRecBytes);
-                        ap_t = a_w[r0.x];
-                        as_t = a_w[r0.y];
-                    }
-                    // ---- positivity (row A3) ------------------------------------------
+                    const double dpv = dd.x, dsv = dd.y, thr = th.x, inv_rho = th.y;
+                    // ---- positivity (row A3): sign bits of rho a_p + delta_p, rho a_s + delta_s
                     const double gn = fma(alpha, g, g);                 // rho * g, exactly rounded
-                    const double ap_new = fma(gn, cap, dd.x);           // rho a_p + delta_p
-                    const double as_new = fma(gn, cas, dd.y);
-                    const bool feas = active && (ap_new >= 0.0) && (as_new >= 0.0);
-                    int fl = feas ? 1 : 0;
+                    const double ap_new = fma(gn, ap_t, dpv);
+                    const double as_new = fma(gn, as_t, dsv);
+                    const bool feas = (__double2hiint(ap_new) | __double2hiint(as_new)) >= 0;
+                    // one walker per warp: an infeasible move skips the tau loop (warp-uniform branch);
+                    // several walkers per warp: always evaluate, infeasible groups just cannot accept
+                    const bool do_eval = (G == 32) ? feas : true;
+                    // ---- incremental Delta chi^2 over all tau (row A4, Eq. 22 + Eq. 9) -------------------
                     double dchi2 = 0.0;
-                    if (__any_sync(0xffffffffu, feas)) {
-                        // ---- incremental Delta chi^2 over all tau (row A4, Eq. 22 + Eq. 9) -----------
-                        double e0p, e0s;
-                        if (P.fact) {
-                            e0p = s_E0[(p >> P.fact_shift) * G + sub] * s_E0[(P.n_hi + (p & fmask)) * G + sub];
-                            e0s = s_E0[(s >> P.fact_shift) * G + sub] * s_E0[(P.n_hi + (s & fmask)) * G + sub];
-                        } else {
-                            e0p = s_E0[p * G + sub];
-                            e0s = s_E0[s * G + sub];
-                        }
-                        double ep = dd.x * e0p, es = dd.y * e0s;
+                    if (do_eval) {
                         double acc_a = 0.0, acc_b = 0.0;
 #pragma unroll
                         for (int i = 0; i < C; ++i) {
-                            const double v = ep + es;
-                            d[i] = fma(alpha, mt[i], v);
+                            d[i] = fma(alpha, mt[i], v[i]);
                             const double t = fma(Wt[i], d[i], G2[i]);
                             if (i & 1) acc_b = fma(d[i], t, acc_b);
                             else       acc_a = fma(d[i], t, acc_a);
-                            if (i + 1 < C) { ep *= rr.x; es *= rr.y; }
                         }
-                        dchi2 = acc_a + acc_b;
+                        dchi2 = (C > 1) ? acc_a + acc_b : acc_a;
+                    }
+                    if (mm + 1 < nb) prepare(mm + 1);                   // overlaps the reduction below
+                    int fl = feas ? 1 : 0;
+                    if (do_eval) {
 #pragma unroll
-                        for (int off = G / 2; off > 0; off >>= 1) dchi2 += shfl_xor_f64(dchi2, off);
+                        for (int off = G / 2; off > 0; off >>= 1) dchi2 += __shfl_xor_sync(0xffffffffu, dchi2, off);
                         fl |= 4;
-                        // ---- Metropolis (row A5, Eq. 10): accept iff dchi2/T + ln u < 0 --------------
-                        const bool acc = feas && (dchi2 < th.x);
+                        // ---- Metropolis (row A5, Eq. 10): accept iff dchi2/T + ln u < 0 ------------------
+                        const bool acc = feas && (dchi2 < thr);
                         if (__any_sync(0xffffffffu, acc)) {
                             if (acc) {
 #pragma unroll
@@ -195,10 +247,10 @@ __global__ void __launch_bounds__(MAXW * 32, 1) sweep_kernel(const SweepArgs P)
                                 }
                                 chi2 += dchi2;
                                 g = gn;
-                                ginv *= th.y;
+                                ginv *= inv_rho;
                                 const double ap_store = ap_new * ginv, as_store = as_new * ginv;
-                                if (sub == 0) { a_w[p] = ap_store; a_w[s] = as_store; }
-                                // the next move's values were fetched before this store
+                                if (leader) { a_w[(unsigned)p] = ap_store; a_w[(unsigned)s] = as_store; }
+                                // the next move's coefficients were fetched before this store
                                 if (r0.x == p) ap_t = ap_store; else if (r0.x == s) ap_t = as_store;
                                 if (r0.y == p) as_t = ap_store; else if (r0.y == s) as_t = as_store;
                                 acc_sweep++;
@@ -207,29 +259,31 @@ __global__ void __launch_bounds__(MAXW * 32, 1) sweep_kernel(const SweepArgs P)
                             __syncwarp();
                         }
                     }
-                    tot_eval += feas ? 1 : 0;
-                    if (sub == 0 && active) {
-                        if (P.flags)
-                            P.flags[((size_t)w * P.call_sweeps + P.call_off + isw) * n_omega + m0 + mm] = (uint8_t)fl;
-                        if (tracing) {
-                            sail_trace_rec *tr = P.trace + (((size_t)(w - P.trace_lo) * P.call_sweeps + P.call_off + isw)
-                                                            * n_omega + m0 + mm);
-                            tr->p = p; tr->s = s; tr->flags = fl; tr->move = m0 + mm;
-                            tr->rho = 1.0 + alpha; tr->delta_p = dd.x; tr->delta_s = dd.y;
-                            tr->dchi2 = dchi2; tr->thr = th.x; tr->ap_new = ap_new; tr->as_new = as_new;
+                    eval_sweep += fl & 1;
+                    if (TRACE) {
+                        if (leader && w < P.W) {
+                            const size_t mv = ((size_t)(P.call_off + isw)) * n_omega + m0 + mm;
+                            if (P.flags) P.flags[(size_t)w * P.call_sweeps * n_omega + mv] = (uint8_t)fl;
+                            if (tracing) {
+                                sail_trace_rec *tr = P.trace + ((size_t)(w - P.trace_lo) * P.call_sweeps * n_omega + mv);
+                                tr->p = p; tr->s = s; tr->flags = fl; tr->move = m0 + mm;
+                                tr->rho = 1.0 + alpha; tr->delta_p = dpv; tr->delta_s = dsv;
+                                tr->dchi2 = dchi2; tr->thr = thr; tr->ap_new = ap_new; tr->as_new = as_new;
+                            }
                         }
                     }
                 }
                 __syncwarp();
             }
 
-            // ---- end of sweep: fold the lazy scale (Eq. 19) and update y (row A6, Eq. 30) ------------
-            if (active) {
-                for (int k = sub; k < n_omega; k += G) a_w[k] *= g;
-            }
+            // ---- end of sweep: fold the lazy scale (Eq. 19), counters, y (row A6, Eq. 30) ------------
+            for (int k = sub; k < n_omega; k += G) a_w[k] *= g;
             g = 1.0;
             ginv = 1.0;
-            tot_acc += acc_sweep;
+            if (leader) {
+                P.n_acc[w] += (unsigned long long)acc_sweep;
+                P.n_eval[w] += (unsigned long long)eval_sweep;
+            }
             if (P.amp_mode == 1) {
                 const double rate = (double)acc_sweep / (double)n_omega;
                 if (rate >= P.amp_p) y = 1.0;
@@ -243,31 +297,30 @@ __global__ void __launch_bounds__(MAXW * 32, 1) sweep_kernel(const SweepArgs P)
         }
 
         // ---- store the state back ----------------------------------------------------------------
-        if (active) {
 #pragma unroll
-            for (int i = 0; i < C; ++i) {
-                const int j = sub + G * i;
-                if (j < P.n_tau) P.mt[(size_t)w * P.n_tau + j] = mt[i];
-            }
-            if (sub == 0) {
-                P.chi2[w] = chi2;
-                P.y[w] = y;
-                P.n_acc[w] += tot_acc;
-                P.n_eval[w] += tot_eval;
-            }
+        for (int i = 0; i < C; ++i) {
+            const int j = sub + G * i;
+            if (j < P.n_tau) P.mt[(size_t)w * P.n_tau + j] = mt[i];
+        }
+        if (leader) {
+            P.chi2[w] = chi2;
+            P.y[w] = y;
         }
         __syncwarp();
     }
 }
 
-// ---- sweep tables: ratio[k] = exp(-omega_k G dtau); start values E0 (direct or factored) -------------
-__global__ void sweep_tables_kernel(int n_omega, int G, double omega0, double domega, double tau0, double dtau,
+// ---- sweep tables: ratio[k] = exp(-omega_k G dtau); invd[k] = 1/(k domega); start values E0 ----------
+__global__ void sweep_tables_kernel(int n_omega, int G, double domega, double tau0, double dtau,
                                     const double *omega, int fact, int shift, int n_hi, int n_lo,
-                                    double *ratio, double *E0)
+                                    double *ratio, double *invd, double *E0)
 {
     const int tid = blockIdx.x * blockDim.x + threadIdx.x;
     const int stride = gridDim.x * blockDim.x;
-    for (int k = tid; k < n_omega; k += stride) ratio[k] = exp(-omega[k] * ((double)G * dtau));
+    for (int k = tid; k < n_omega; k += stride) {
+        ratio[k] = exp(-omega[k] * ((double)G * dtau));
+        invd[k] = k ? 1.0 / ((double)k * domega) : 0.0;
+    }
     if (!fact) {
         for (int i = tid; i < n_omega * G; i += stride) {
             const int k = i / G, l = i % G;
@@ -280,6 +333,17 @@ __global__ void sweep_tables_kernel(int n_omega, int G, double omega0, double do
             // high part carries omega_0; low part the remaining k_lo * domega
             E0[i] = (r < n_hi) ? exp(-omega[(size_t)r << shift] * t) : exp(-((double)(r - n_hi) * domega) * t);
         }
+    }
+}
+
+// scratch walker slots W .. W_pad-1 := copies of walker W-1
+__global__ void pad_walkers_kernel(int n_omega, int n_tau, long long W, long long W_pad, double *a, double *mt,
+                                   double *chi2, double *y)
+{
+    for (long long r = W + blockIdx.x; r < W_pad; r += gridDim.x) {
+        for (int k = threadIdx.x; k < n_omega; k += blockDim.x) a[(size_t)r * n_omega + k] = a[(size_t)(W - 1) * n_omega + k];
+        for (int j = threadIdx.x; j < n_tau; j += blockDim.x) mt[(size_t)r * n_tau + j] = mt[(size_t)(W - 1) * n_tau + j];
+        if (threadIdx.x == 0) { chi2[r] = chi2[W - 1]; y[r] = y[W - 1]; }
     }
 }
 
@@ -297,16 +361,15 @@ int ensure_sweep_tables(sail_handle *h, int G)
     }
     h->tables_fact = fact;
     h->fact_shift = shift;
-    sweep_tables_kernel<<<64, 256, 0, h->stream>>>(h->n_omega, G, h->omega0, h->domega, h->tau0, h->dtau,
-                                                   h->tab.omega, fact ? 1 : 0, shift, n_hi, n_lo,
-                                                   h->sw_ratio, h->sw_E0);
+    sweep_tables_kernel<<<64, 256, 0, h->stream>>>(h->n_omega, G, h->domega, h->tau0, h->dtau, h->tab.omega,
+                                                   fact ? 1 : 0, shift, n_hi, n_lo, h->sw_ratio, h->sw_invd, h->sw_E0);
     SAIL_LAUNCH_OK(h, "sweep_tables_kernel");
     h->tables_G = G;
     return SAIL_OK;
 }
 
 // ---- dispatch -----------------------------------------------------------------------------------------
-template <int G, int C, int MAXW>
+template <int G, int C, int MAXW, bool FACT, bool TRACE>
 static int launch_variant(sail_handle *h, SweepArgs &args)
 {
     constexpr int NW = 32 / G;
@@ -317,12 +380,16 @@ static int launch_variant(sail_handle *h, SweepArgs &args)
     long long ctas = (args.n_groups + warps - 1) / warps;
     if (ctas > h->num_sms) ctas = h->num_sms;
     const int e0_elems = args.fact ? (args.n_hi + args.n_lo) * G : args.n_omega * G;
-    const size_t smem = (size_t)(((args.n_omega + 1) & ~1) + ((e0_elems + 1) & ~1)) * sizeof(double)
+    const size_t smem = (size_t)(3 * ((args.n_omega + 1) & ~1) + ((e0_elems + 1) & ~1)) * sizeof(double)
                         + (size_t)warps * 32 * kRecBytes;
     if (smem > 227 * 1024)
         return set_err(h, SAIL_ERR_ARG, "sweep tables need %zu bytes of shared memory (> 227 KB)", smem);
-    auto kern = sweep_kernel<G, C, MAXW>;
+    auto kern = sweep_kernel<G, C, MAXW, FACT, TRACE>;
     SAIL_CUDA_OK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    int resident = 0;
+    SAIL_CUDA_OK(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, warps * 32, smem));
+    if (resident < 1)
+        return set_err(h, SAIL_ERR_CUDA, "sweep_kernel<%d,%d,%d> does not fit one SM at %d warps per CTA", G, C, MAXW, warps);
     kern<<<(unsigned)ctas, warps * 32, smem, h->stream>>>(args);
     SAIL_LAUNCH_OK(h, "sweep_kernel");
     return SAIL_OK;
@@ -336,7 +403,7 @@ static int pick_lanes(const sail_handle *h, int requested)
     for (int G = 8; G <= 32; G *= 2) {
         const int C = (h->n_tau + G - 1) / G;
         const long long warps = (h->W * G + 31) / 32;
-        if (C <= 16 && warps >= (long long)h->num_sms * 24) return G;
+        if (C <= 16 && warps >= (long long)h->num_sms * 12) return G;
     }
     return 32;
 }
@@ -349,13 +416,19 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     if (C > 16) return set_err(h, SAIL_ERR_ARG, "n_tau=%d needs more than 16 tau-points per lane at %d lanes", h->n_tau, G);
     int rc = ensure_sweep_tables(h, G);
     if (rc) return rc;
+    const long long W_pad = (h->W + 3) & ~3LL;
+    if (W_pad > h->W) {
+        pad_walkers_kernel<<<(unsigned)(W_pad - h->W), 128, 0, h->stream>>>(h->n_omega, h->n_tau, h->W, W_pad, h->st.a,
+                                                                          h->st.mt, h->st.chi2, h->st.y);
+        SAIL_LAUNCH_OK(h, "pad_walkers_kernel");
+    }
 
     SweepArgs a{};
     a.n_omega = h->n_omega; a.n_tau = h->n_tau; a.W = h->W;
-    a.A = h->A; a.B = h->B; a.domega = h->domega; a.eta = p->eta;
+    a.A = h->A; a.B = h->B; a.omega_mid0 = h->omega0 + 0.5 * h->domega; a.domega = h->domega; a.eta = p->eta;
     a.amp_p = p->amp_p; a.amp_m = p->amp_m; a.y_min = p->y_min; a.amp_mode = p->amp_mode;
     a.seed_lo = (uint32_t)(h->seed & 0xFFFFFFFFu); a.seed_hi = (uint32_t)(h->seed >> 32);
-    a.omega = h->tab.omega; a.Wj = h->tab.Wj; a.fj = h->tab.fj; a.ratio = h->sw_ratio; a.E0 = h->sw_E0;
+    a.Wj = h->tab.Wj; a.fj = h->tab.fj; a.ratio = h->sw_ratio; a.E0 = h->sw_E0; a.invd = h->sw_invd; a.omega = h->tab.omega;
     a.fact = h->tables_fact ? 1 : 0; a.fact_shift = h->fact_shift;
     if (h->tables_fact) { a.n_lo = 1 << h->fact_shift; a.n_hi = (h->n_omega + a.n_lo - 1) >> h->fact_shift; }
     a.a = h->st.a; a.mt = h->st.mt; a.chi2 = h->st.chi2; a.y = h->st.y;
@@ -363,13 +436,18 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     a.T = d_T; a.sweep0 = h->sweep; a.n_sweeps = (int)n_sweeps;
     a.trace_lo = p->trace_lo; a.trace_hi = p->trace_hi; a.trace = p->trace; a.flags = p->flags;
     a.call_sweeps = sweeps_in_call; a.call_off = call_offset;
+    const bool trace = (p->trace != nullptr) || (p->flags != nullptr);
 
-#define SAIL_VARIANT(GG, CC, MW) if (G == GG && C <= CC) return launch_variant<GG, CC, MW>(h, a);
-    SAIL_VARIANT(32, 1, 28) SAIL_VARIANT(32, 2, 28) SAIL_VARIANT(32, 4, 28)
-    SAIL_VARIANT(32, 7, 16) SAIL_VARIANT(32, 8, 16) SAIL_VARIANT(32, 16, 10)
-    SAIL_VARIANT(16, 2, 28) SAIL_VARIANT(16, 4, 28) SAIL_VARIANT(16, 7, 16)
-    SAIL_VARIANT(16, 8, 16) SAIL_VARIANT(16, 13, 10) SAIL_VARIANT(16, 16, 10)
-    SAIL_VARIANT(8, 4, 28) SAIL_VARIANT(8, 8, 16) SAIL_VARIANT(8, 13, 10) SAIL_VARIANT(8, 16, 10)
+#define SAIL_VARIANT(GG, CC, MW)                                                                         \
+    if (G == GG && C <= CC) {                                                                            \
+        if (a.fact) return trace ? launch_variant<GG, CC, MW, true, true>(h, a) : launch_variant<GG, CC, MW, true, false>(h, a);   \
+        return trace ? launch_variant<GG, CC, MW, false, true>(h, a) : launch_variant<GG, CC, MW, false, false>(h, a);             \
+    }
+    SAIL_VARIANT(32, 1, 16) SAIL_VARIANT(32, 2, 16) SAIL_VARIANT(32, 4, 16)
+    SAIL_VARIANT(32, 7, 12) SAIL_VARIANT(32, 8, 12) SAIL_VARIANT(32, 16, 8)
+    SAIL_VARIANT(16, 2, 16) SAIL_VARIANT(16, 4, 16) SAIL_VARIANT(16, 7, 14)
+    SAIL_VARIANT(16, 8, 12) SAIL_VARIANT(16, 13, 8) SAIL_VARIANT(16, 16, 8)
+    SAIL_VARIANT(8, 4, 16) SAIL_VARIANT(8, 8, 12) SAIL_VARIANT(8, 13, 8) SAIL_VARIANT(8, 16, 8)
 #undef SAIL_VARIANT
     return set_err(h, SAIL_ERR_ARG, "no sweep kernel variant for lanes=%d, tau-points per lane=%d", G, C);
 }
