@@ -72,6 +72,70 @@ __device__ __forceinline__ int4 lds_s32x4(uint32_t addr)
     return v;
 }
 
+// element pointer a + idx (idx < 2^32) in one IMAD.WIDE
+__device__ __forceinline__ double *elem_ptr(double *base, int idx)
+{
+    unsigned long long r;
+    asm("mad.wide.u32 %0, %1, 8, %2;" : "=l"(r) : "r"(idx), "l"(reinterpret_cast<unsigned long long>(base)));
+    return reinterpret_cast<double *>(r);
+}
+// predicated (not branched) FP64 updates: lanes of walkers that did not accept keep their state without
+// the warp diverging
+__device__ __forceinline__ void add_if(double &x, double y, int pred)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %2, 0;\n\t@p add.rn.f64 %0, %0, %1;\n\t}" : "+d"(x) : "d"(y), "r"(pred));
+}
+__device__ __forceinline__ void fma_if(double &x, double a, double b, int pred)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %3, 0;\n\t@p fma.rn.f64 %0, %1, %2, %0;\n\t}" : "+d"(x) : "d"(a), "d"(b), "r"(pred));
+}
+__device__ __forceinline__ void mul_if(double &x, double a, int pred)
+{
+    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %2, 0;\n\t@p mul.rn.f64 %0, %0, %1;\n\t}" : "+d"(x) : "d"(a), "r"(pred));
+}
+
+
+// ---- one proposal (row A2): Philox4x32-10 keyed by (seed; walker, sweep, move, 0) -> 64-byte record ------
+//   [ 0] p, s (int32), alpha = rho - 1      [16] delta_p, delta_s (Eq. 20-21)
+//   [32] thr = -T ln u_acc, 1/rho            [48] exp(-omega_p G dtau), exp(-omega_s G dtau)
+__device__ __forceinline__ void propose(const SweepArgs &P, uint32_t walker, uint32_t sweep, uint32_t move, double y, double T,
+                                        const double *s_ratio, const double *s_invd, const double *s_wm, unsigned char *rec)
+{
+    uint32_t x[4];
+    philox4x32_10(walker, sweep, move, 0u, P.seed_lo, P.seed_hi, x);
+    const int p = (int)__umulhi(x[0], (uint32_t)P.n_omega);
+    int s = (int)__umulhi(x[1], (uint32_t)(P.n_omega - 1));
+    s += (s >= p) ? 1 : 0;
+    const double u_rho = ((double)x[2] + 0.5) * 2.3283064365386962890625e-10;
+    const double u_acc = ((double)x[3] + 0.5) * 2.3283064365386962890625e-10;
+    // rho in the method's operation order, no contraction: bit-identical to the definition
+    const double rho = __dsub_rn(1.0, __dmul_rn(__dmul_rn(y, P.eta), __dsub_rn(__dmul_rn(2.0, u_rho), 1.0)));
+    const double alpha = __dsub_rn(rho, 1.0);          // exact
+    // Eq. 20-21 in the method's operation order; only the division by (p-s) domega is a multiplication by
+    // the correctly rounded reciprocal (delta within 2 ulp of the division form)
+    const double omr = __dsub_rn(1.0, rho);
+    const int dps = p - s;
+    const double inv = (dps > 0) ? s_invd[dps] : -s_invd[-dps];
+    const double dp = __dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[s]))), inv);
+    const double ds = -__dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[p]))), inv);
+    const double thr = -T * log(u_acc);
+    *reinterpret_cast<int4 *>(rec) = make_int4(p, s, __double2loint(alpha), __double2hiint(alpha));
+    *reinterpret_cast<double2 *>(rec + 16) = make_double2(dp, ds);
+    *reinterpret_cast<double2 *>(rec + 32) = make_double2(thr, fast_recip(rho));
+    *reinterpret_cast<double2 *>(rec + 48) = make_double2(s_ratio[p], s_ratio[s]);
+}
+
+// Eq. 30: y from the sweep's acceptance rate
+__device__ __forceinline__ double amp_factor(const SweepArgs &P, int acc_sweep, double y)
+{
+    if (P.amp_mode != 1) return y;
+    const double rate = (double)acc_sweep / (double)P.n_omega;
+    if (rate >= P.amp_p) return 1.0;
+    const double x = rate / P.amp_p;
+    const double yy = (P.amp_m == 2.0) ? x * x : pow(x, P.amp_m);
+    return yy < P.y_min ? P.y_min : yy;
+}
+
 // MAXW = warps per CTA (one CTA per SM) the variant is register-budgeted for; the register file is allocated in
 // units of 4 warps per CTA, so the budget is 65536 / (roundup4(MAXW) * 32) registers per thread.
 // FACT: start values E0[k][l] = H[k_hi][l] * L[k_lo][l] (two small tables) instead of one N_omega x G table.
@@ -146,31 +210,8 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
             for (int m0 = 0; m0 < n_omega; m0 += G) {
                 const int nb = min(G, n_omega - m0);
                 // ---- proposals for moves m0 .. m0+nb-1, one per lane (row A2) -----------------------
-                if (sub < nb) {
-                    uint32_t x[4];
-                    philox4x32_10((uint32_t)w, sweep, (uint32_t)(m0 + sub), 0u, P.seed_lo, P.seed_hi, x);
-                    const int p = (int)__umulhi(x[0], (uint32_t)n_omega);
-                    int s = (int)__umulhi(x[1], (uint32_t)(n_omega - 1));
-                    s += (s >= p) ? 1 : 0;
-                    const double u_rho = ((double)x[2] + 0.5) * 2.3283064365386962890625e-10;
-                    const double u_acc = ((double)x[3] + 0.5) * 2.3283064365386962890625e-10;
-                    // rho in the method's operation order, no contraction: bit-identical to the definition
-                    const double rho = __dsub_rn(1.0, __dmul_rn(__dmul_rn(y, P.eta),
-                                                                __dsub_rn(__dmul_rn(2.0, u_rho), 1.0)));
-                    const double alpha = __dsub_rn(rho, 1.0);          // exact
-                    // Eq. 20-21 in the method's operation order; only the division by (p-s) domega is a
-                    // multiplication by the correctly rounded reciprocal (delta within 2 ulp of the division)
-                    const double omr = __dsub_rn(1.0, rho);
-                    const int dps = p - s;
-                    const double inv = (dps > 0) ? s_invd[dps] : -s_invd[-dps];
-                    const double dp = __dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[s]))), inv);
-                    const double ds = -__dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[p]))), inv);
-                    const double thr = -P.T[isw] * log(u_acc);
-                    *reinterpret_cast<int4 *>(my_rec_w) = make_int4(p, s, __double2loint(alpha), __double2hiint(alpha));
-                    *reinterpret_cast<double2 *>(my_rec_w + 16) = make_double2(dp, ds);
-                    *reinterpret_cast<double2 *>(my_rec_w + 32) = make_double2(thr, fast_recip(rho));
-                    *reinterpret_cast<double2 *>(my_rec_w + 48) = make_double2(s_ratio[p], s_ratio[s]);
-                }
+                if (sub < nb)
+                    propose(P, (uint32_t)w, sweep, (uint32_t)(m0 + sub), y, P.T[isw], s_ratio, s_invd, s_wm, my_rec_w);
                 __syncwarp();
 
                 // ---- software pipeline -------------------------------------------------------------------
@@ -186,8 +227,8 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                     dd = lds_f64x2(r + 16);
                     th = lds_f64x2(r + 32);
                     const double2 rr = lds_f64x2(r + 48);
-                    ap_t = a_w[(unsigned)r0.x];
-                    as_t = a_w[(unsigned)r0.y];
+                    ap_t = *elem_ptr(a_w, r0.x);
+                    as_t = *elem_ptr(a_w, r0.y);
                     double e0p, e0s;
                     if (FACT) {
                         e0p = lds_f64(e0_lane + (uint32_t)((r0.x >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.x & fmask) * (G * 8)));
@@ -196,11 +237,16 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                         e0p = lds_f64(e0_lane + (uint32_t)(r0.x * (G * 8)));
                         e0s = lds_f64(e0_lane + (uint32_t)(r0.y * (G * 8)));
                     }
-                    double ep = dd.x * e0p, es = dd.y * e0s;
+                    // geometric recurrence, two interleaved sub-chains per row (even / odd i) to halve its depth
+                    double ep0 = dd.x * e0p, es0 = dd.y * e0s;
+                    double ep1 = ep0 * rr.x, es1 = es0 * rr.y;
+                    const double rp2 = rr.x * rr.x, rs2 = rr.y * rr.y;
 #pragma unroll
-                    for (int i = 0; i < C; ++i) {
-                        v[i] = ep + es;
-                        if (i + 1 < C) { ep *= rr.x; es *= rr.y; }
+                    for (int i = 0; i < C; i += 2) {
+                        v[i] = ep0 + es0;
+                        if (i + 1 < C) v[i + 1] = ep1 + es1;
+                        if (i + 2 < C) { ep0 *= rp2; es0 *= rs2; }
+                        if (i + 3 < C) { ep1 *= rp2; es1 *= rs2; }
                     }
                 };
                 prepare(0);
@@ -230,7 +276,9 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                         }
                         dchi2 = (C > 1) ? acc_a + acc_b : acc_a;
                     }
-                    if (mm + 1 < nb) prepare(mm + 1);                   // overlaps the reduction below
+                    // prepare the next move (clamped: the last step re-prepares
+                    // itself, harmlessly) — no branch, so the scheduler can interleave it with the reduction below
+                    prepare(min(mm + 1, nb - 1));
                     int fl = feas ? 1 : 0;
                     if (do_eval) {
 #pragma unroll
@@ -239,23 +287,24 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                         // ---- Metropolis (row A5, Eq. 10): accept iff dchi2/T + ln u < 0 ------------------
                         const bool acc = feas && (dchi2 < thr);
                         if (__any_sync(0xffffffffu, acc)) {
-                            if (acc) {
+                            const int ia = acc ? 1 : 0;
 #pragma unroll
-                                for (int i = 0; i < C; ++i) {
-                                    mt[i] += d[i];
-                                    G2[i] = fma(Wt[i], d[i] + d[i], G2[i]);
-                                }
-                                chi2 += dchi2;
-                                g = gn;
-                                ginv *= inv_rho;
-                                const double ap_store = ap_new * ginv, as_store = as_new * ginv;
-                                if (leader) { a_w[(unsigned)p] = ap_store; a_w[(unsigned)s] = as_store; }
-                                // the next move's coefficients were fetched before this store
+                            for (int i = 0; i < C; ++i) {
+                                add_if(mt[i], d[i], ia);
+                                fma_if(G2[i], Wt[i], d[i] + d[i], ia);
+                            }
+                            add_if(chi2, dchi2, ia);
+                            g = acc ? gn : g;
+                            mul_if(ginv, inv_rho, ia);
+                            const double ap_store = ap_new * ginv, as_store = as_new * ginv;
+                            if (leader && acc) { *elem_ptr(a_w, p) = ap_store; *elem_ptr(a_w, s) = as_store; }
+                            // the next move's coefficients were fetched before this store
+                            if (acc) {
                                 if (r0.x == p) ap_t = ap_store; else if (r0.x == s) ap_t = as_store;
                                 if (r0.y == p) as_t = ap_store; else if (r0.y == s) as_t = as_store;
-                                acc_sweep++;
-                                fl |= 2;
                             }
+                            acc_sweep += ia;
+                            fl |= ia << 1;
                             __syncwarp();
                         }
                     }
@@ -284,15 +333,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                 P.n_acc[w] += (unsigned long long)acc_sweep;
                 P.n_eval[w] += (unsigned long long)eval_sweep;
             }
-            if (P.amp_mode == 1) {
-                const double rate = (double)acc_sweep / (double)n_omega;
-                if (rate >= P.amp_p) y = 1.0;
-                else {
-                    const double x = rate / P.amp_p;
-                    const double yy = (P.amp_m == 2.0) ? x * x : pow(x, P.amp_m);
-                    y = yy < P.y_min ? P.y_min : yy;
-                }
-            }
+            y = amp_factor(P, acc_sweep, y);
             __syncwarp();
         }
 
@@ -306,6 +347,161 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
             P.chi2[w] = chi2;
             P.y[w] = y;
         }
+        __syncwarp();
+    }
+}
+
+
+// ---- one walker per WARP, register-lean (<= 72 registers: 28 resident warps per SM = 7 per sub-partition) ------
+// Same arithmetic as sweep_kernel<32, C, ...>; no software pipeline (the other six warps of the sub-partition hide
+// the latencies), every decision is warp-uniform, so infeasible and rejected moves branch around the work.
+template <int C, int MAXW, bool FACT, bool TRACE>
+__global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kernel_warp(const SweepArgs P)
+{
+    constexpr int G = 32;
+    extern __shared__ __align__(16) unsigned char smem[];
+    double *s_ratio = reinterpret_cast<double *>(smem);
+    const int n_omega = P.n_omega;
+    const int n_omega_pad = (n_omega + 1) & ~1;
+    double *s_invd = s_ratio + n_omega_pad;
+    double *s_wm = s_invd + n_omega_pad;
+    double *s_E0 = s_wm + n_omega_pad;
+    const int e0_elems = FACT ? (P.n_hi + P.n_lo) * G : n_omega * G;
+    unsigned char *s_recs = reinterpret_cast<unsigned char *>(s_E0 + ((e0_elems + 1) & ~1));
+    for (int i = threadIdx.x; i < n_omega; i += blockDim.x) {
+        s_ratio[i] = P.ratio[i]; s_invd[i] = P.invd[i]; s_wm[i] = __dadd_rn(P.omega[i], 0.5 * P.domega);
+    }
+    for (int i = threadIdx.x; i < e0_elems; i += blockDim.x) s_E0[i] = P.E0[i];
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    unsigned char *my_rec_w = s_recs + ((size_t)warp * 32 + lane) * kRecBytes;
+    const uint32_t rbase = (uint32_t)__cvta_generic_to_shared(s_recs) + (uint32_t)(warp * 32 * kRecBytes);
+    const uint32_t e0_lane = (uint32_t)__cvta_generic_to_shared(s_E0) + (uint32_t)(lane * 8);
+    const uint32_t e0_lo = e0_lane + (uint32_t)(P.n_hi * G * 8);
+    const int warps_per_cta = blockDim.x >> 5;
+    const int fshift = P.fact_shift;
+    const int fmask = (1 << fshift) - 1;
+
+    for (long long w = (long long)blockIdx.x * warps_per_cta + warp; w < P.n_groups; w += (long long)gridDim.x * warps_per_cta) {
+        double *__restrict__ a_w = P.a + (size_t)w * n_omega;
+        double mt[C], G2[C], Wt[C], d[C];
+#pragma unroll
+        for (int i = 0; i < C; ++i) {
+            const int j = lane + G * i;
+            const bool ok = j < P.n_tau;
+            mt[i] = ok ? P.mt[(size_t)w * P.n_tau + j] : 0.0;
+            Wt[i] = ok ? P.Wj[j] : 0.0;
+            d[i] = 0.0;
+        }
+        double chi2 = P.chi2[w];
+        double g = 1.0, ginv = 1.0;
+        bool tracing = false;
+        if (TRACE) tracing = P.trace != nullptr && w >= P.trace_lo && w < P.trace_hi;
+
+        for (int isw = 0; isw < P.n_sweeps; ++isw) {
+            int acc_sweep = 0, eval_sweep = 0;
+#pragma unroll
+            for (int i = 0; i < C; ++i) {
+                const int j = lane + G * i;
+                const double f = (j < P.n_tau) ? P.fj[j] : 0.0;
+                G2[i] = 2.0 * Wt[i] * (mt[i] - f);
+            }
+            for (int m0 = 0; m0 < n_omega; m0 += G) {
+                const int nb = min(G, n_omega - m0);
+                if (lane < nb)
+                    propose(P, (uint32_t)w, (uint32_t)(P.sweep0 + isw), (uint32_t)(m0 + lane), P.y[w], P.T[isw],
+                            s_ratio, s_invd, s_wm, my_rec_w);
+                __syncwarp();
+                for (int mm = 0; mm < nb; ++mm) {
+                    const uint32_t r = rbase + (uint32_t)(mm * kRecBytes);
+                    const int4 r0 = lds_s32x4(r);
+                    const double2 dd = lds_f64x2(r + 16);
+                    const double alpha = __hiloint2double(r0.w, r0.z);
+                    // ---- positivity (row A3) ----------------------------------------------
+                    const double gn = fma(alpha, g, g);
+                    const double ap_new = fma(gn, a_w[(unsigned)r0.x], dd.x);
+                    const double as_new = fma(gn, a_w[(unsigned)r0.y], dd.y);
+                    const bool feas = (__double2hiint(ap_new) | __double2hiint(as_new)) >= 0;
+                    int fl = 0;
+                    double dchi2 = 0.0;
+                    if (feas) {
+                        // ---- incremental Delta chi^2 over all tau (row A4, Eq. 22 + Eq. 9) ---------------
+                        const double2 rr = lds_f64x2(r + 48);
+                        double ep, es;
+                        if (FACT) {
+                            ep = lds_f64(e0_lane + (uint32_t)((r0.x >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.x & fmask) * (G * 8)));
+                            es = lds_f64(e0_lane + (uint32_t)((r0.y >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.y & fmask) * (G * 8)));
+                        } else {
+                            ep = lds_f64(e0_lane + (uint32_t)(r0.x * (G * 8)));
+                            es = lds_f64(e0_lane + (uint32_t)(r0.y * (G * 8)));
+                        }
+                        ep *= dd.x;
+                        es *= dd.y;
+                        double acc_a = 0.0, acc_b = 0.0;
+#pragma unroll
+                        for (int i = 0; i < C; ++i) {
+                            d[i] = fma(alpha, mt[i], ep + es);
+                            const double t = fma(Wt[i], d[i], G2[i]);
+                            if (i & 1) acc_b = fma(d[i], t, acc_b);
+                            else       acc_a = fma(d[i], t, acc_a);
+                            if (i + 1 < C) { ep *= rr.x; es *= rr.y; }
+                        }
+                        dchi2 = (C > 1) ? acc_a + acc_b : acc_a;
+#pragma unroll
+                        for (int off = 16; off > 0; off >>= 1) dchi2 += __shfl_xor_sync(0xffffffffu, dchi2, off);
+                        fl = 5;
+                        eval_sweep++;
+                        // ---- Metropolis (row A5, Eq. 10); identical in every lane: a uniform branch ------
+                        const double2 th = lds_f64x2(r + 32);
+                        if (dchi2 < th.x) {
+#pragma unroll
+                            for (int i = 0; i < C; ++i) {
+                                mt[i] += d[i];
+                                G2[i] = fma(Wt[i], d[i] + d[i], G2[i]);
+                            }
+                            chi2 += dchi2;
+                            g = gn;
+                            ginv *= th.y;
+                            if (lane == 0) { a_w[(unsigned)r0.x] = ap_new * ginv; a_w[(unsigned)r0.y] = as_new * ginv; }
+                            acc_sweep++;
+                            fl = 7;
+                            __syncwarp();
+                        }
+                    }
+                    if (TRACE) {
+                        if (lane == 0 && w < P.W) {
+                            const size_t mv = ((size_t)(P.call_off + isw)) * n_omega + m0 + mm;
+                            if (P.flags) P.flags[(size_t)w * P.call_sweeps * n_omega + mv] = (uint8_t)fl;
+                            if (tracing) {
+                                sail_trace_rec *tr = P.trace + ((size_t)(w - P.trace_lo) * P.call_sweeps * n_omega + mv);
+                                tr->p = r0.x; tr->s = r0.y; tr->flags = fl; tr->move = m0 + mm;
+                                tr->rho = 1.0 + alpha; tr->delta_p = dd.x; tr->delta_s = dd.y;
+                                tr->dchi2 = dchi2; tr->thr = lds_f64(r + 32); tr->ap_new = ap_new; tr->as_new = as_new;
+                            }
+                        }
+                    }
+                }
+                __syncwarp();
+            }
+            // ---- end of sweep: fold the lazy scale (Eq. 19), counters, y (row A6, Eq. 30) ----------------
+            for (int k = lane; k < n_omega; k += G) a_w[k] *= g;
+            g = 1.0;
+            ginv = 1.0;
+            if (lane == 0) {
+                P.n_acc[w] += (unsigned long long)acc_sweep;
+                P.n_eval[w] += (unsigned long long)eval_sweep;
+                P.y[w] = amp_factor(P, acc_sweep, P.y[w]);
+            }
+            __syncwarp();
+        }
+#pragma unroll
+        for (int i = 0; i < C; ++i) {
+            const int j = lane + G * i;
+            if (j < P.n_tau) P.mt[(size_t)w * P.n_tau + j] = mt[i];
+        }
+        if (lane == 0) P.chi2[w] = chi2;
         __syncwarp();
     }
 }
@@ -369,7 +565,7 @@ int ensure_sweep_tables(sail_handle *h, int G)
 }
 
 // ---- dispatch -----------------------------------------------------------------------------------------
-template <int G, int C, int MAXW, bool FACT, bool TRACE>
+template <int G, int C, int MAXW, bool FACT, bool TRACE, bool LEAN = false>
 static int launch_variant(sail_handle *h, SweepArgs &args)
 {
     constexpr int NW = 32 / G;
@@ -384,7 +580,9 @@ static int launch_variant(sail_handle *h, SweepArgs &args)
                         + (size_t)warps * 32 * kRecBytes;
     if (smem > 227 * 1024)
         return set_err(h, SAIL_ERR_ARG, "sweep tables need %zu bytes of shared memory (> 227 KB)", smem);
-    auto kern = sweep_kernel<G, C, MAXW, FACT, TRACE>;
+    void (*kern)(const SweepArgs);
+    if constexpr (LEAN) kern = sweep_kernel_warp<C, MAXW, FACT, TRACE>;
+    else kern = sweep_kernel<G, C, MAXW, FACT, TRACE>;
     SAIL_CUDA_OK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int resident = 0;
     SAIL_CUDA_OK(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, warps * 32, smem));
@@ -397,6 +595,7 @@ static int launch_variant(sail_handle *h, SweepArgs &args)
 
 static int pick_lanes(const sail_handle *h, int requested)
 {
+    if (requested == 33) return 32;      // tuning: software-pipelined 32-lane variant instead of the lean one
     if (requested == 8 || requested == 16 || requested == 32) return requested;
     // auto: fewest lanes per walker that (a) keep <= 16 tau-points per lane and (b) still leave
     // enough warps to fill every SM sub-partition several times over
@@ -443,6 +642,8 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
         if (a.fact) return trace ? launch_variant<GG, CC, MW, true, true>(h, a) : launch_variant<GG, CC, MW, true, false>(h, a);   \
         return trace ? launch_variant<GG, CC, MW, false, true>(h, a) : launch_variant<GG, CC, MW, false, false>(h, a);             \
     }
+    if (G == 32 && C <= 4 && !a.fact && p->lanes_per_walker != 33)   // one walker per warp, register-lean: 28 warps per SM
+        return trace ? launch_variant<32, 4, 28, false, true, true>(h, a) : launch_variant<32, 4, 28, false, false, true>(h, a);
     SAIL_VARIANT(32, 1, 16) SAIL_VARIANT(32, 2, 16) SAIL_VARIANT(32, 4, 16)
     SAIL_VARIANT(32, 7, 12) SAIL_VARIANT(32, 8, 12) SAIL_VARIANT(32, 16, 8)
     SAIL_VARIANT(16, 2, 16) SAIL_VARIANT(16, 4, 16) SAIL_VARIANT(16, 7, 14)
