@@ -73,11 +73,22 @@ __device__ __forceinline__ int4 lds_s32x4(uint32_t addr)
 }
 
 // element pointer a + idx (idx < 2^32) in one IMAD.WIDE
-__device__ __forceinline__ double *elem_ptr(double *base, int idx)
+__device__ __forceinline__ double *elem_ptr(double *base, uint32_t idx)
 {
     unsigned long long r;
     asm("mad.wide.u32 %0, %1, 8, %2;" : "=l"(r) : "r"(idx), "l"(reinterpret_cast<unsigned long long>(base)));
     return reinterpret_cast<double *>(r);
+}
+__device__ __forceinline__ double ldg_f64(const double *p)
+{
+    double v;
+    asm volatile("ld.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+    return v;
+}
+// predicated (not branched) store: only the lanes with pred != 0 write
+__device__ __forceinline__ void stg_f64_if(double *p, double v, int pred)
+{
+    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %2, 0;\n\t@q st.global.f64 [%0], %1;\n\t}" :: "l"(p), "d"(v), "r"(pred) : "memory");
 }
 // predicated (not branched) FP64 updates: lanes of walkers that did not accept keep their state without
 // the warp diverging
@@ -227,8 +238,8 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                     dd = lds_f64x2(r + 16);
                     th = lds_f64x2(r + 32);
                     const double2 rr = lds_f64x2(r + 48);
-                    ap_t = *elem_ptr(a_w, r0.x);
-                    as_t = *elem_ptr(a_w, r0.y);
+                    ap_t = ldg_f64(elem_ptr(a_w, (uint32_t)r0.x));
+                    as_t = ldg_f64(elem_ptr(a_w, (uint32_t)r0.y));
                     double e0p, e0s;
                     if (FACT) {
                         e0p = lds_f64(e0_lane + (uint32_t)((r0.x >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.x & fmask) * (G * 8)));
@@ -297,7 +308,8 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                             g = acc ? gn : g;
                             mul_if(ginv, inv_rho, ia);
                             const double ap_store = ap_new * ginv, as_store = as_new * ginv;
-                            if (leader && acc) { *elem_ptr(a_w, p) = ap_store; *elem_ptr(a_w, s) = as_store; }
+                            stg_f64_if(elem_ptr(a_w, (uint32_t)p), ap_store, (leader && acc) ? 1 : 0);
+                            stg_f64_if(elem_ptr(a_w, (uint32_t)s), as_store, (leader && acc) ? 1 : 0);
                             // the next move's coefficients were fetched before this store
                             if (acc) {
                                 if (r0.x == p) ap_t = ap_store; else if (r0.x == s) ap_t = as_store;
@@ -377,15 +389,22 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
     unsigned char *my_rec_w = s_recs + ((size_t)warp * 32 + lane) * kRecBytes;
-    const uint32_t rbase = (uint32_t)__cvta_generic_to_shared(s_recs) + (uint32_t)(warp * 32 * kRecBytes);
-    const uint32_t e0_lane = (uint32_t)__cvta_generic_to_shared(s_E0) + (uint32_t)(lane * 8);
+    // 32-bit shared-window addresses, made opaque so that they stay in registers instead of being
+    // rematerialised (the generic->shared conversion costs an S2R + several ALU instructions per move)
+    uint32_t rbase = (uint32_t)__cvta_generic_to_shared(s_recs) + (uint32_t)(warp * 32 * kRecBytes);
+    uint32_t e0_lane = (uint32_t)__cvta_generic_to_shared(s_E0) + (uint32_t)(lane * 8);
+    asm volatile("" : "+r"(rbase), "+r"(e0_lane));
     const uint32_t e0_lo = e0_lane + (uint32_t)(P.n_hi * G * 8);
     const int warps_per_cta = blockDim.x >> 5;
     const int fshift = P.fact_shift;
     const int fmask = (1 << fshift) - 1;
+    const int lane0 = (lane == 0) ? 1 : 0;
 
     for (long long w = (long long)blockIdx.x * warps_per_cta + warp; w < P.n_groups; w += (long long)gridDim.x * warps_per_cta) {
-        double *__restrict__ a_w = P.a + (size_t)w * n_omega;
+        // element offset of this walker's spectrum: the whole spectra array has < 2^32 elements (checked at launch)
+        uint32_t wbase = (uint32_t)(w * n_omega);
+        asm volatile("" : "+r"(wbase));
+        double *const a_all = P.a;
         double mt[C], G2[C], Wt[C], d[C];
 #pragma unroll
         for (int i = 0; i < C; ++i) {
@@ -414,29 +433,34 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                     propose(P, (uint32_t)w, (uint32_t)(P.sweep0 + isw), (uint32_t)(m0 + lane), P.y[w], P.T[isw],
                             s_ratio, s_invd, s_wm, my_rec_w);
                 __syncwarp();
-                for (int mm = 0; mm < nb; ++mm) {
-                    const uint32_t r = rbase + (uint32_t)(mm * kRecBytes);
+                const uint32_t r_end = rbase + (uint32_t)(nb * kRecBytes);
+                for (uint32_t r = rbase; r != r_end; r += kRecBytes) {
                     const int4 r0 = lds_s32x4(r);
                     const double2 dd = lds_f64x2(r + 16);
                     const double alpha = __hiloint2double(r0.w, r0.z);
+                    double *const pp = elem_ptr(a_all, wbase + (uint32_t)r0.x);
+                    double *const ps = elem_ptr(a_all, wbase + (uint32_t)r0.y);
+                    const double a_p = ldg_f64(pp), a_s = ldg_f64(ps);
+                    // issued before the feasibility branch so that their latency overlaps the positivity test
+                    const double2 rr = lds_f64x2(r + 48);
+                    const double2 th = lds_f64x2(r + 32);
+                    double ep, es;
+                    if (FACT) {
+                        ep = lds_f64(e0_lane + (uint32_t)((r0.x >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.x & fmask) * (G * 8)));
+                        es = lds_f64(e0_lane + (uint32_t)((r0.y >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.y & fmask) * (G * 8)));
+                    } else {
+                        ep = lds_f64(e0_lane + (uint32_t)(r0.x * (G * 8)));
+                        es = lds_f64(e0_lane + (uint32_t)(r0.y * (G * 8)));
+                    }
                     // ---- positivity (row A3) ----------------------------------------------
                     const double gn = fma(alpha, g, g);
-                    const double ap_new = fma(gn, a_w[(unsigned)r0.x], dd.x);
-                    const double as_new = fma(gn, a_w[(unsigned)r0.y], dd.y);
+                    const double ap_new = fma(gn, a_p, dd.x);
+                    const double as_new = fma(gn, a_s, dd.y);
                     const bool feas = (__double2hiint(ap_new) | __double2hiint(as_new)) >= 0;
                     int fl = 0;
                     double dchi2 = 0.0;
                     if (feas) {
                         // ---- incremental Delta chi^2 over all tau (row A4, Eq. 22 + Eq. 9) ---------------
-                        const double2 rr = lds_f64x2(r + 48);
-                        double ep, es;
-                        if (FACT) {
-                            ep = lds_f64(e0_lane + (uint32_t)((r0.x >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.x & fmask) * (G * 8)));
-                            es = lds_f64(e0_lane + (uint32_t)((r0.y >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.y & fmask) * (G * 8)));
-                        } else {
-                            ep = lds_f64(e0_lane + (uint32_t)(r0.x * (G * 8)));
-                            es = lds_f64(e0_lane + (uint32_t)(r0.y * (G * 8)));
-                        }
                         ep *= dd.x;
                         es *= dd.y;
                         double acc_a = 0.0, acc_b = 0.0;
@@ -454,7 +478,6 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                         fl = 5;
                         eval_sweep++;
                         // ---- Metropolis (row A5, Eq. 10); identical in every lane: a uniform branch ------
-                        const double2 th = lds_f64x2(r + 32);
                         if (dchi2 < th.x) {
 #pragma unroll
                             for (int i = 0; i < C; ++i) {
@@ -464,7 +487,8 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                             chi2 += dchi2;
                             g = gn;
                             ginv *= th.y;
-                            if (lane == 0) { a_w[(unsigned)r0.x] = ap_new * ginv; a_w[(unsigned)r0.y] = as_new * ginv; }
+                            stg_f64_if(pp, ap_new * ginv, lane0);
+                            stg_f64_if(ps, as_new * ginv, lane0);
                             acc_sweep++;
                             fl = 7;
                             __syncwarp();
@@ -472,13 +496,14 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                     }
                     if (TRACE) {
                         if (lane == 0 && w < P.W) {
+                            const int mm = (int)((r - rbase) / kRecBytes);
                             const size_t mv = ((size_t)(P.call_off + isw)) * n_omega + m0 + mm;
                             if (P.flags) P.flags[(size_t)w * P.call_sweeps * n_omega + mv] = (uint8_t)fl;
                             if (tracing) {
                                 sail_trace_rec *tr = P.trace + ((size_t)(w - P.trace_lo) * P.call_sweeps * n_omega + mv);
                                 tr->p = r0.x; tr->s = r0.y; tr->flags = fl; tr->move = m0 + mm;
                                 tr->rho = 1.0 + alpha; tr->delta_p = dd.x; tr->delta_s = dd.y;
-                                tr->dchi2 = dchi2; tr->thr = lds_f64(r + 32); tr->ap_new = ap_new; tr->as_new = as_new;
+                                tr->dchi2 = dchi2; tr->thr = th.x; tr->ap_new = ap_new; tr->as_new = as_new;
                             }
                         }
                     }
@@ -486,7 +511,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                 __syncwarp();
             }
             // ---- end of sweep: fold the lazy scale (Eq. 19), counters, y (row A6, Eq. 30) ----------------
-            for (int k = lane; k < n_omega; k += G) a_w[k] *= g;
+            for (int k = lane; k < n_omega; k += G) a_all[(size_t)wbase + k] *= g;
             g = 1.0;
             ginv = 1.0;
             if (lane == 0) {
@@ -616,6 +641,8 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     int rc = ensure_sweep_tables(h, G);
     if (rc) return rc;
     const long long W_pad = (h->W + 3) & ~3LL;
+    if ((unsigned long long)W_pad * (unsigned long long)h->n_omega >= (1ull << 32))
+        return set_err(h, SAIL_ERR_ARG, "W * n_omega must be < 2^32 spectral coefficients");
     if (W_pad > h->W) {
         pad_walkers_kernel<<<(unsigned)(W_pad - h->W), 128, 0, h->stream>>>(h->n_omega, h->n_tau, h->W, W_pad, h->st.a,
                                                                           h->st.mt, h->st.chi2, h->st.y);
