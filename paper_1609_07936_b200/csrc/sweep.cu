@@ -622,13 +622,9 @@ static int pick_lanes(const sail_handle *h, int requested)
 {
     if (requested == 33) return 32;      // tuning: software-pipelined 32-lane variant instead of the lean one
     if (requested == 8 || requested == 16 || requested == 32) return requested;
-    // auto: fewest lanes per walker that (a) keep <= 16 tau-points per lane and (b) still leave
-    // enough warps to fill every SM sub-partition several times over
-    for (int G = 8; G <= 32; G *= 2) {
-        const int C = (h->n_tau + G - 1) / G;
-        const long long warps = (h->W * G + 31) / 32;
-        if (C <= 16 && warps >= (long long)h->num_sms * 12) return G;
-    }
+    // auto: one walker per warp.  Measured on B200 (profiles/): the register-lean 32-lane kernel beats the
+    // sub-warp (8 / 16 lanes per walker) software-pipelined variants on all five workloads, because residency
+    // (warps per sub-partition) matters more than per-move scalar overhead for this serial-latency-bound chain.
     return 32;
 }
 
@@ -669,8 +665,14 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
         if (a.fact) return trace ? launch_variant<GG, CC, MW, true, true>(h, a) : launch_variant<GG, CC, MW, true, false>(h, a);   \
         return trace ? launch_variant<GG, CC, MW, false, true>(h, a) : launch_variant<GG, CC, MW, false, false>(h, a);             \
     }
-    if (G == 32 && C <= 4 && !a.fact && p->lanes_per_walker != 33)   // one walker per warp, register-lean: 28 warps per SM
-        return trace ? launch_variant<32, 4, 28, false, true, true>(h, a) : launch_variant<32, 4, 28, false, false, true>(h, a);
+    // one walker per warp, register-lean (the default at 32 lanes; lanes_per_walker = 33 selects the pipelined form)
+#define SAIL_LEAN(CC, MW)                                                                                        \
+    if (G == 32 && C <= CC && p->lanes_per_walker != 33) {                                                       \
+        if (a.fact) return trace ? launch_variant<32, CC, MW, true, true, true>(h, a) : launch_variant<32, CC, MW, true, false, true>(h, a);   \
+        return trace ? launch_variant<32, CC, MW, false, true, true>(h, a) : launch_variant<32, CC, MW, false, false, true>(h, a);             \
+    }
+    SAIL_LEAN(4, 28) SAIL_LEAN(8, 16) SAIL_LEAN(16, 12)
+#undef SAIL_LEAN
     SAIL_VARIANT(32, 1, 16) SAIL_VARIANT(32, 2, 16) SAIL_VARIANT(32, 4, 16)
     SAIL_VARIANT(32, 7, 12) SAIL_VARIANT(32, 8, 12) SAIL_VARIANT(32, 16, 8)
     SAIL_VARIANT(16, 2, 16) SAIL_VARIANT(16, 4, 16) SAIL_VARIANT(16, 7, 14)
