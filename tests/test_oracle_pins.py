@@ -433,3 +433,31 @@ def test_branch_imprint_t1_copies_and_t_preserves_sum_rules(tiny):
             M = oracle.forward(o.K, o.a[i])
             np.testing.assert_array_equal(o.M[i], M)
             assert o.chi2[i] == oracle.chi2(M, tiny.F, tiny.sigma)
+
+
+# ----------------------------------------------------------------------------- regression fixture
+def test_oracle_reproduces_its_committed_trace():
+    """tests/golden/oracle_tiny_trace.txt is written by tests/golden/make_oracle_golden.py from the oracle alone;
+    integer fields must match exactly, floating fields to 1e-13 (libm exp/log may differ in the last bit
+    between machines)."""
+    sys_path = os.path.join(GOLDEN, "make_oracle_golden.py")
+    import importlib.util
+    spec = importlib.util.spec_from_file_location("make_oracle_golden", sys_path)
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    _, chi2_0, tr, o = mod.compute()
+    n = 0
+    for line in open(os.path.join(GOLDEN, "oracle_tiny_trace.txt")):
+        if line.startswith("# chi2_0"):
+            vals = [float(x) for x in line.split()[2:]]
+            np.testing.assert_allclose(chi2_0, vals, rtol=1e-12)
+        if line.startswith("#"):
+            continue
+        f = line.split()
+        wk, sw, m = int(f[0]), int(f[1]), int(f[2])
+        t = tr[wk, sw, m]
+        assert (t["p"], t["s"], t["flags"]) == (int(f[3]), int(f[4]), int(f[5]))
+        for name, val in zip(("rho", "delta_p", "delta_s", "dchi2", "ln_u"), f[6:11]):
+            assert float(t[name]) == pytest.approx(float(val), rel=1e-11, abs=1e-300), name
+        n += 1
+    assert n == 96
