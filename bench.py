@@ -94,6 +94,10 @@ def measured_peaks():
         return {}
 
 
+# dram__bytes_read.sum + dram__bytes_write.sum of one sweep-kernel launch, from the committed ncu --set full capture
+# (profiles/r01_sweep_small_full_metrics.txt): 12.09 MB + 2.35 MB for the whole 5000-sweep Small anneal
+SWEEP_DRAM_BYTES_PER_LAUNCH = {("small", 5000): 14.44e6}
+
 LANES = 0   # --lanes: lanes of a warp per walker (0 = library default)
 
 
@@ -240,7 +244,7 @@ def main_ours(args):
         algo_instr_per_launch = DFMA_PER_TAU_POINT * w.n_tau * evaluated / max(n_sweep_launches / args.steps, 1)
         achieved = DFMA_PER_TAU_POINT * w.n_tau * evaluated * args.steps / kern_total
         roofline = {"bound": "alu", "kernel": "sail::sweep_kernel", "achieved": achieved / 1e12, "peak": peak_nominal / 1e12,
-                    "unit": "T FP64 lane-instr/s", "frac": achieved / peak_nominal, "traffic": None,
+                    "unit": "T FP64 lane-instr/s", "frac": achieved / peak_nominal, "traffic": SWEEP_DRAM_BYTES_PER_LAUNCH.get((w.name, w.n_sweeps)),
                     "peak_source": f"derived: {num_sms} SMs x {FP64_LANES_PER_SM} FP64 lanes x {sm_max:.0f} MHz (DESIGN.md §7)",
                     "peak_measured_dfma": dfma_measured / 1e12, "frac_of_measured_dfma": achieved / dfma_measured,
                     "algorithmic_instr_per_launch": algo_instr_per_launch,

@@ -278,6 +278,40 @@ def test_bench_configuration_sampled_parity():
     s.close()
 
 
+def test_stress_configuration_sampled_parity():
+    """configs[4] (Throughput stress) at FULL size (W = 262144, N_omega = 2048, N_tau = 512; 5.4 GB of state; factored
+    start tables, 16 tau-points per lane, 12 warps per SM): one sweep, 8 sampled walkers from the far end of the
+    population traced on the GPU and replayed by the oracle from the injected state; then one branching event whose
+    multipliers must sum to W."""
+    w = wl.make("stress", simpson_intervals=100_000)
+    s = _sail(w, w.W)
+    s.init_walkers(w.W, w.A, w.B, SEED)
+    lo, hi = 262100, 262108
+    a_g, c_g = s.get()
+    o = _oracle(w, hi - lo, spectra=a_g[lo:hi])
+    np.testing.assert_allclose(o.chi2, c_g[lo:hi], rtol=1e-7)
+    o.chi2[:] = c_g[lo:hi]
+    del a_g
+    T = w.schedule[:1]
+    tg, _ = s.anneal(T, w.eta, trace_walkers=(lo, hi))
+    tr_o = np.zeros((hi - lo, 1, w.n_omega), dtype=oracle.TRACE_DTYPE)
+    for i in range(hi - lo):
+        for m in range(w.n_omega):
+            tr_o[i, 0, m] = _oracle_move(o, i, lo + i, 0, m, T[0])
+    assert compare_traces(tg, tr_o, T, w.A / w.n_omega) == 0
+    a2, c2 = s.get()
+    np.testing.assert_allclose(a2[lo:hi], o.a, rtol=0, atol=1e-10 * o.a.max())
+    np.testing.assert_allclose(c2[lo:hi], o.chi2, rtol=1e-9)
+    info, mult, donor = s.branch(float(np.std(c2)), 0.1, want_maps=True)
+    assert mult.sum() == w.W and info.n_recipients == (mult == 0).sum() == np.maximum(mult - 1, 0).sum()
+    rec = np.where(donor >= 0)[0]
+    assert (mult[donor[rec]] >= 2).all() and (np.diff(donor[rec]) >= 0).all()
+    a3, _ = s.get()
+    i = rec[len(rec) // 2]
+    np.testing.assert_array_equal(a3[i], 0.1 * a2[donor[i]] + (1.0 - 0.1) * a2[i])
+    s.close()
+
+
 def _oracle_move(o, local, walker_id, sweep, move, T):
     """orc_move with an explicit Philox walker id (the oracle object holds only the sampled walkers)."""
     import ctypes as C
