@@ -357,7 +357,7 @@ if __name__ == "__main__":
     ap.add_argument("--sweeps", type=int, default=0, help="override the number of sweeps (debug)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--extra", type=int, default=1, help="also time a block of the stress config (N=1 only)")
-    ap.add_argument("--lanes", type=int, default=0, help="lanes per walker: 0 auto, 8, 16, 32")
+    ap.add_argument("--lanes", type=int, default=0, help="lanes per walker / kernel form: 0 auto, 8, 16, 32..35 (include/sail.h)")
     a = ap.parse_args()
     LANES = a.lanes
     sys.exit(main_reference(a) if a.impl == "reference" else main_ours(a))

@@ -531,6 +531,240 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
     }
 }
 
+// ---- one walker per WARP, feasibility-screened ("mask") form: the default ------------------------------------
+// Differences from sweep_kernel_warp (same moves, same decisions):
+//  * positivity (row A3) is tested for all moves of a 32-move batch AT ONCE, one move per lane, against the
+//    current spectrum: a ballot gives the mask of feasible moves and the serial chain visits only those — an
+//    infeasible move costs nothing.  Every accepted move changes the spectrum (all coefficients scale by rho,
+//    two of them shift), so the lanes behind it are screened again; the values a lane holds from its LAST
+//    screen are exactly rho a_p + delta_p, rho a_s + delta_s of the state at its turn.
+//  * the kernel-row combination v_i = delta_p E_p,i + delta_s E_s,i (i = tau-point index of the lane) obeys
+//    the two-term linear recurrence of its two geometric modes,
+//        v_{i+1} = (r_p + r_s) v_i - (r_p r_s) v_{i-1},      r_k = exp(-omega_k 32 dtau),
+//    so the tau loop costs 5 FP64 instructions per tau-point (DMUL + DFMA for v, then the three DFMAs of
+//    d, W d + G2, d (W d + G2)): the algorithmic count of SURVEY §8d.  Rounding errors enter relative to |v_i|
+//    and propagate through the bounded Green's function (r_p^{n+1} - r_s^{n+1})/(r_p - r_s) <= n + 1.
+//  * with W2REG the constants 2 Wj live in registers as well: the accepted update is 2 instructions per
+//    tau-point instead of 3.
+constexpr int kRecMaskBytes = 80;
+// record: [0] p, s (int32), alpha = rho - 1   [16] delta_p, delta_s   [32] delta_p r_p, delta_s r_s
+//         [48] r_p + r_s, -(r_p r_s)          [64] thr = -T ln u_acc, 1/rho
+__device__ __forceinline__ void propose_mask(const SweepArgs &P, uint32_t walker, uint32_t sweep, uint32_t move, double y, double T,
+                                             const double *s_ratio, const double *s_invd, const double *s_wm, unsigned char *rec)
+{
+    uint32_t x[4];
+    philox4x32_10(walker, sweep, move, 0u, P.seed_lo, P.seed_hi, x);
+    const int p = (int)__umulhi(x[0], (uint32_t)P.n_omega);
+    int s = (int)__umulhi(x[1], (uint32_t)(P.n_omega - 1));
+    s += (s >= p) ? 1 : 0;
+    const double u_rho = ((double)x[2] + 0.5) * 2.3283064365386962890625e-10;
+    const double u_acc = ((double)x[3] + 0.5) * 2.3283064365386962890625e-10;
+    const double rho = __dsub_rn(1.0, __dmul_rn(__dmul_rn(y, P.eta), __dsub_rn(__dmul_rn(2.0, u_rho), 1.0)));
+    const double alpha = __dsub_rn(rho, 1.0);
+    const double omr = __dsub_rn(1.0, rho);
+    const int dps = p - s;
+    const double inv = (dps > 0) ? s_invd[dps] : -s_invd[-dps];
+    const double dp = __dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[s]))), inv);
+    const double ds = -__dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[p]))), inv);
+    const double thr = -T * log(u_acc);
+    const double rp = s_ratio[p], rs = s_ratio[s];
+    *reinterpret_cast<int4 *>(rec) = make_int4(p, s, __double2loint(alpha), __double2hiint(alpha));
+    *reinterpret_cast<double2 *>(rec + 16) = make_double2(dp, ds);
+    *reinterpret_cast<double2 *>(rec + 32) = make_double2(dp * rp, ds * rs);
+    *reinterpret_cast<double2 *>(rec + 48) = make_double2(rp + rs, -(rp * rs));
+    *reinterpret_cast<double2 *>(rec + 64) = make_double2(thr, fast_recip(rho));
+}
+
+template <int C, int MAXW, bool FACT, bool TRACE, bool W2REG>
+__global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kernel_mask(const SweepArgs P)
+{
+    constexpr int G = 32;
+    extern __shared__ __align__(16) unsigned char smem[];
+    double *s_ratio = reinterpret_cast<double *>(smem);
+    const int n_omega = P.n_omega;
+    const int n_omega_pad = (n_omega + 1) & ~1;
+    double *s_invd = s_ratio + n_omega_pad;
+    double *s_wm = s_invd + n_omega_pad;
+    double *s_E0 = s_wm + n_omega_pad;
+    const int e0_elems = FACT ? (P.n_hi + P.n_lo) * G : n_omega * G;
+    unsigned char *s_recs = reinterpret_cast<unsigned char *>(s_E0 + ((e0_elems + 1) & ~1));
+    for (int i = threadIdx.x; i < n_omega; i += blockDim.x) {
+        s_ratio[i] = P.ratio[i]; s_invd[i] = P.invd[i]; s_wm[i] = __dadd_rn(P.omega[i], 0.5 * P.domega);
+    }
+    for (int i = threadIdx.x; i < e0_elems; i += blockDim.x) s_E0[i] = P.E0[i];
+    // records of lanes beyond a short last batch are read (and masked out) by the screen: keep p = s = 0 there
+    for (int i = threadIdx.x; i < (int)(blockDim.x * (kRecMaskBytes / 4)); i += blockDim.x)
+        reinterpret_cast<uint32_t *>(s_recs)[i] = 0u;
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    unsigned char *my_rec_w = s_recs + ((size_t)warp * 32 + lane) * kRecMaskBytes;
+    uint32_t rbase = (uint32_t)__cvta_generic_to_shared(s_recs) + (uint32_t)(warp * 32 * kRecMaskBytes);
+    uint32_t e0_lane = (uint32_t)__cvta_generic_to_shared(s_E0) + (uint32_t)(lane * 8);
+    asm volatile("" : "+r"(rbase), "+r"(e0_lane));
+    const uint32_t rec_own = rbase + (uint32_t)(lane * kRecMaskBytes);
+    const uint32_t e0_lo = e0_lane + (uint32_t)(P.n_hi * G * 8);
+    const int warps_per_cta = blockDim.x >> 5;
+    const int fshift = P.fact_shift;
+    const int fmask = (1 << fshift) - 1;
+
+    for (long long w = (long long)blockIdx.x * warps_per_cta + warp; w < P.n_groups; w += (long long)gridDim.x * warps_per_cta) {
+        uint32_t wbase = (uint32_t)(w * n_omega);
+        asm volatile("" : "+r"(wbase));
+        double *const a_all = P.a;
+        double mt[C], G2[C], Wt[C], d[C], W2[W2REG ? C : 1];
+#pragma unroll
+        for (int i = 0; i < C; ++i) {
+            const int j = lane + G * i;
+            const bool ok = j < P.n_tau;
+            mt[i] = ok ? P.mt[(size_t)w * P.n_tau + j] : 0.0;
+            Wt[i] = ok ? P.Wj[j] : 0.0;
+            if (W2REG) W2[i] = Wt[i] + Wt[i];
+            d[i] = 0.0;
+        }
+        double chi2 = P.chi2[w];
+        double g = 1.0, ginv = 1.0;
+        bool tracing = false;
+        if (TRACE) tracing = P.trace != nullptr && w >= P.trace_lo && w < P.trace_hi;
+
+        for (int isw = 0; isw < P.n_sweeps; ++isw) {
+            int acc_sweep = 0, eval_sweep = 0;
+#pragma unroll
+            for (int i = 0; i < C; ++i) {
+                const int j = lane + G * i;
+                const double f = (j < P.n_tau) ? P.fj[j] : 0.0;
+                G2[i] = 2.0 * Wt[i] * (mt[i] - f);
+            }
+            const double y_sweep = P.y[w];
+            const double T_sweep = P.T[isw];
+            for (int m0 = 0; m0 < n_omega; m0 += G) {
+                const int nb = min(G, n_omega - m0);
+                if (lane < nb)
+                    propose_mask(P, (uint32_t)w, (uint32_t)(P.sweep0 + isw), (uint32_t)(m0 + lane), y_sweep, T_sweep,
+                                 s_ratio, s_invd, s_wm, my_rec_w);
+                __syncwarp();
+                const uint32_t valid = (nb == 32) ? 0xffffffffu : ((1u << nb) - 1u);
+
+                // ---- positivity screen (row A3), one move per lane --------------------------
+                double apn = 0.0, asn = 0.0;          // rho a_p + delta_p, rho a_s + delta_s of this lane's move
+                auto screen = [&](uint32_t sel) -> uint32_t {
+                    const int4 q0 = lds_s32x4(rec_own);
+                    const double2 qd = lds_f64x2(rec_own + 16);
+                    const double a_p = ldg_f64(elem_ptr(a_all, wbase + (uint32_t)q0.x));
+                    const double a_s = ldg_f64(elem_ptr(a_all, wbase + (uint32_t)q0.y));
+                    const double qa = __hiloint2double(q0.w, q0.z);
+                    const double gn = fma(qa, g, g);
+                    const double x_p = fma(gn, a_p, qd.x);
+                    const double x_s = fma(gn, a_s, qd.y);
+                    if (!TRACE || ((sel >> lane) & 1u)) { apn = x_p; asn = x_s; }
+                    const bool feas = (__double2hiint(x_p) | __double2hiint(x_s)) >= 0;
+                    return __ballot_sync(0xffffffffu, feas) & sel;
+                };
+                uint32_t mask = screen(valid);
+                uint32_t tr_eval = 0u, tr_acc = 0u;   // TRACE: moves evaluated / accepted in this batch
+                double tr_dchi2 = 0.0;
+
+                while (mask) {
+                    const int m = __ffs((int)mask) - 1;
+                    const uint32_t r = rbase + (uint32_t)(m * kRecMaskBytes);
+                    const int4 r0 = lds_s32x4(r);
+                    const double2 dd = lds_f64x2(r + 16);
+                    const double2 dr = lds_f64x2(r + 32);
+                    const double2 sc = lds_f64x2(r + 48);
+                    const double2 th = lds_f64x2(r + 64);
+                    const double alpha = __hiloint2double(r0.w, r0.z);
+                    double e0p, e0s;
+                    if (FACT) {
+                        e0p = lds_f64(e0_lane + (uint32_t)((r0.x >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.x & fmask) * (G * 8)));
+                        e0s = lds_f64(e0_lane + (uint32_t)((r0.y >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.y & fmask) * (G * 8)));
+                    } else {
+                        e0p = lds_f64(e0_lane + (uint32_t)(r0.x * (G * 8)));
+                        e0s = lds_f64(e0_lane + (uint32_t)(r0.y * (G * 8)));
+                    }
+                    // ---- incremental Delta chi^2 over all tau (row A4, Eq. 22 + Eq. 9) -------------------
+                    double vm = fma(dd.x, e0p, dd.y * e0s);        // v_0
+                    double vc = fma(dr.x, e0p, dr.y * e0s);        // v_1
+                    double acc_a = 0.0, acc_b = 0.0;
+#pragma unroll
+                    for (int i = 0; i < C; ++i) {
+                        double vi;
+                        if (i == 0) vi = vm;
+                        else if (i == 1) vi = vc;
+                        else { vi = fma(sc.x, vc, sc.y * vm); vm = vc; vc = vi; }
+                        d[i] = fma(alpha, mt[i], vi);
+                        const double t = fma(Wt[i], d[i], G2[i]);
+                        if (i & 1) acc_b = fma(d[i], t, acc_b);
+                        else       acc_a = fma(d[i], t, acc_a);
+                    }
+                    double dchi2 = (C > 1) ? acc_a + acc_b : acc_a;
+#pragma unroll
+                    for (int off = 16; off > 0; off >>= 1) dchi2 += __shfl_xor_sync(0xffffffffu, dchi2, off);
+                    eval_sweep++;
+                    if (TRACE) { tr_eval |= 1u << m; if (lane == m) tr_dchi2 = dchi2; }
+                    // ---- Metropolis (row A5, Eq. 10); identical in every lane: a uniform branch ----------
+                    if (dchi2 < th.x) {
+#pragma unroll
+                        for (int i = 0; i < C; ++i) {
+                            mt[i] += d[i];
+                            if (W2REG) G2[i] = fma(W2[i], d[i], G2[i]);
+                            else       G2[i] = fma(Wt[i], d[i] + d[i], G2[i]);
+                        }
+                        chi2 += dchi2;
+                        g = fma(alpha, g, g);
+                        ginv *= th.y;
+                        const int mine = (lane == m) ? 1 : 0;
+                        stg_f64_if(elem_ptr(a_all, wbase + (uint32_t)r0.x), apn * ginv, mine);
+                        stg_f64_if(elem_ptr(a_all, wbase + (uint32_t)r0.y), asn * ginv, mine);
+                        acc_sweep++;
+                        if (TRACE) tr_acc |= 1u << m;
+                        __syncwarp();
+                        // the spectrum changed: screen the moves behind this one again
+                        mask = screen(valid & ~((2u << m) - 1u));
+                    } else {
+                        mask &= mask - 1u;
+                    }
+                }
+                if (TRACE) {
+                    if (lane < nb && w < P.W) {
+                        const int4 q0 = lds_s32x4(rec_own);
+                        const double2 qd = lds_f64x2(rec_own + 16);
+                        const double2 qt = lds_f64x2(rec_own + 64);
+                        const bool feas = (__double2hiint(apn) | __double2hiint(asn)) >= 0;
+                        const int fl = (feas ? 1 : 0) | (((tr_acc >> lane) & 1u) ? 2 : 0) | (((tr_eval >> lane) & 1u) ? 4 : 0);
+                        const size_t mv = ((size_t)(P.call_off + isw)) * n_omega + m0 + lane;
+                        if (P.flags) P.flags[(size_t)w * P.call_sweeps * n_omega + mv] = (uint8_t)fl;
+                        if (tracing) {
+                            sail_trace_rec *tr = P.trace + ((size_t)(w - P.trace_lo) * P.call_sweeps * n_omega + mv);
+                            tr->p = q0.x; tr->s = q0.y; tr->flags = fl; tr->move = m0 + lane;
+                            tr->rho = 1.0 + __hiloint2double(q0.w, q0.z); tr->delta_p = qd.x; tr->delta_s = qd.y;
+                            tr->dchi2 = tr_dchi2; tr->thr = qt.x; tr->ap_new = apn; tr->as_new = asn;
+                        }
+                    }
+                }
+                __syncwarp();
+            }
+            // ---- end of sweep: fold the lazy scale (Eq. 19), counters, y (row A6, Eq. 30) ----------------
+            for (int k = lane; k < n_omega; k += G) a_all[(size_t)wbase + k] *= g;
+            g = 1.0;
+            ginv = 1.0;
+            if (lane == 0) {
+                P.n_acc[w] += (unsigned long long)acc_sweep;
+                P.n_eval[w] += (unsigned long long)eval_sweep;
+                P.y[w] = amp_factor(P, acc_sweep, y_sweep);
+            }
+            __syncwarp();
+        }
+#pragma unroll
+        for (int i = 0; i < C; ++i) {
+            const int j = lane + G * i;
+            if (j < P.n_tau) P.mt[(size_t)w * P.n_tau + j] = mt[i];
+        }
+        if (lane == 0) P.chi2[w] = chi2;
+        __syncwarp();
+    }
+}
+
 // ---- sweep tables: ratio[k] = exp(-omega_k G dtau); invd[k] = 1/(k domega); start values E0 ----------
 __global__ void sweep_tables_kernel(int n_omega, int G, double domega, double tau0, double dtau,
                                     const double *omega, int fact, int shift, int n_hi, int n_lo,
@@ -590,10 +824,13 @@ int ensure_sweep_tables(sail_handle *h, int G)
 }
 
 // ---- dispatch -----------------------------------------------------------------------------------------
-template <int G, int C, int MAXW, bool FACT, bool TRACE, bool LEAN = false>
+// MODE 0: sub-warp groups / software pipeline (sweep_kernel), 1: lean one walker per warp (sweep_kernel_warp),
+//      2: screened one walker per warp (sweep_kernel_mask), 3: the same with 2 Wj in registers
+template <int G, int C, int MAXW, bool FACT, bool TRACE, int MODE = 0>
 static int launch_variant(sail_handle *h, SweepArgs &args)
 {
     constexpr int NW = 32 / G;
+    constexpr int rec_bytes = (MODE >= 2) ? kRecMaskBytes : kRecBytes;
     args.n_groups = (args.W + NW - 1) / NW;
     int warps = (int)((args.n_groups + h->num_sms - 1) / h->num_sms);
     if (warps > MAXW) warps = MAXW;
@@ -602,36 +839,39 @@ static int launch_variant(sail_handle *h, SweepArgs &args)
     if (ctas > h->num_sms) ctas = h->num_sms;
     const int e0_elems = args.fact ? (args.n_hi + args.n_lo) * G : args.n_omega * G;
     const size_t smem = (size_t)(3 * ((args.n_omega + 1) & ~1) + ((e0_elems + 1) & ~1)) * sizeof(double)
-                        + (size_t)warps * 32 * kRecBytes;
+                        + (size_t)warps * 32 * rec_bytes;
     if (smem > 227 * 1024)
         return set_err(h, SAIL_ERR_ARG, "sweep tables need %zu bytes of shared memory (> 227 KB)", smem);
     void (*kern)(const SweepArgs);
-    if constexpr (LEAN) kern = sweep_kernel_warp<C, MAXW, FACT, TRACE>;
+    if constexpr (MODE == 3) kern = sweep_kernel_mask<C, MAXW, FACT, TRACE, true>;
+    else if constexpr (MODE == 2) kern = sweep_kernel_mask<C, MAXW, FACT, TRACE, false>;
+    else if constexpr (MODE == 1) kern = sweep_kernel_warp<C, MAXW, FACT, TRACE>;
     else kern = sweep_kernel<G, C, MAXW, FACT, TRACE>;
     SAIL_CUDA_OK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int resident = 0;
     SAIL_CUDA_OK(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, warps * 32, smem));
     if (resident < 1)
-        return set_err(h, SAIL_ERR_CUDA, "sweep_kernel<%d,%d,%d> does not fit one SM at %d warps per CTA", G, C, MAXW, warps);
+        return set_err(h, SAIL_ERR_CUDA, "sweep kernel (mode %d, G=%d, C=%d, MAXW=%d) does not fit one SM at %d warps per CTA", MODE, G, C, MAXW, warps);
     kern<<<(unsigned)ctas, warps * 32, smem, h->stream>>>(args);
     SAIL_LAUNCH_OK(h, "sweep_kernel");
     return SAIL_OK;
 }
 
-static int pick_lanes(const sail_handle *h, int requested)
+// lanes_per_walker (a tuning knob, see include/sail.h): 0 / 32 = screened one-walker-per-warp kernel (default),
+// 34 = the unscreened lean form, 33 = software-pipelined form, 8 / 16 = sub-warp groups
+static int pick_lanes(int requested)
 {
-    if (requested == 33) return 32;      // tuning: software-pipelined 32-lane variant instead of the lean one
-    if (requested == 8 || requested == 16 || requested == 32) return requested;
-    // auto: one walker per warp.  Measured on B200 (profiles/): the register-lean 32-lane kernel beats the
-    // sub-warp (8 / 16 lanes per walker) software-pipelined variants on all five workloads, because residency
-    // (warps per sub-partition) matters more than per-move scalar overhead for this serial-latency-bound chain.
+    if (requested == 8 || requested == 16) return requested;
     return 32;
 }
 
 int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sail_anneal_params *p,
                   int64_t sweeps_in_call, int64_t call_offset)
 {
-    const int G = pick_lanes(h, p->lanes_per_walker);
+    const int req = p->lanes_per_walker;
+    if (!(req == 0 || req == 8 || req == 16 || (req >= 32 && req <= 35)))
+        return set_err(h, SAIL_ERR_ARG, "lanes_per_walker=%d is not one of 0, 8, 16, 32..35", req);
+    const int G = pick_lanes(req);
     const int C = (h->n_tau + G - 1) / G;
     if (C > 16) return set_err(h, SAIL_ERR_ARG, "n_tau=%d needs more than 16 tau-points per lane at %d lanes", h->n_tau, G);
     int rc = ensure_sweep_tables(h, G);
@@ -660,26 +900,42 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     a.call_sweeps = sweeps_in_call; a.call_off = call_offset;
     const bool trace = (p->trace != nullptr) || (p->flags != nullptr);
 
-#define SAIL_VARIANT(GG, CC, MW)                                                                         \
-    if (G == GG && C <= CC) {                                                                            \
-        if (a.fact) return trace ? launch_variant<GG, CC, MW, true, true>(h, a) : launch_variant<GG, CC, MW, true, false>(h, a);   \
-        return trace ? launch_variant<GG, CC, MW, false, true>(h, a) : launch_variant<GG, CC, MW, false, false>(h, a);             \
+#define SAIL_VARIANT(GG, CC, MW, MODE)                                                                                  \
+    {                                                                                                                   \
+        if (a.fact) return trace ? launch_variant<GG, CC, MW, true, true, MODE>(h, a) : launch_variant<GG, CC, MW, true, false, MODE>(h, a);   \
+        return trace ? launch_variant<GG, CC, MW, false, true, MODE>(h, a) : launch_variant<GG, CC, MW, false, false, MODE>(h, a);             \
     }
-    // one walker per warp, register-lean (the default at 32 lanes; lanes_per_walker = 33 selects the pipelined form)
-#define SAIL_LEAN(CC, MW)                                                                                        \
-    if (G == 32 && C <= CC && p->lanes_per_walker != 33) {                                                       \
-        if (a.fact) return trace ? launch_variant<32, CC, MW, true, true, true>(h, a) : launch_variant<32, CC, MW, true, false, true>(h, a);   \
-        return trace ? launch_variant<32, CC, MW, false, true, true>(h, a) : launch_variant<32, CC, MW, false, false, true>(h, a);             \
+    if (G == 32 && (req == 0 || req == 32)) {          // screened (default)
+        if (C <= 4) SAIL_VARIANT(32, 4, 28, 2)
+        if (C <= 7) SAIL_VARIANT(32, 7, 16, 3)
+        if (C <= 8) SAIL_VARIANT(32, 8, 16, 3)
+        SAIL_VARIANT(32, 16, 12, 2)
     }
-    SAIL_LEAN(4, 28) SAIL_LEAN(8, 16) SAIL_LEAN(16, 12)
-#undef SAIL_LEAN
-    SAIL_VARIANT(32, 1, 16) SAIL_VARIANT(32, 2, 16) SAIL_VARIANT(32, 4, 16)
-    SAIL_VARIANT(32, 7, 12) SAIL_VARIANT(32, 8, 12) SAIL_VARIANT(32, 16, 8)
-    SAIL_VARIANT(16, 2, 16) SAIL_VARIANT(16, 4, 16) SAIL_VARIANT(16, 7, 14)
-    SAIL_VARIANT(16, 8, 12) SAIL_VARIANT(16, 13, 8) SAIL_VARIANT(16, 16, 8)
-    SAIL_VARIANT(8, 4, 16) SAIL_VARIANT(8, 8, 12) SAIL_VARIANT(8, 13, 8) SAIL_VARIANT(8, 16, 8)
+    if (G == 32 && req == 35) {                        // screened, the other register trade-off
+        if (C <= 4) SAIL_VARIANT(32, 4, 24, 3)
+        if (C <= 7) SAIL_VARIANT(32, 7, 16, 2)
+        if (C <= 8) SAIL_VARIANT(32, 8, 16, 2)
+        SAIL_VARIANT(32, 16, 8, 3)
+    }
+    if (G == 32 && req == 34) {                        // unscreened lean form
+        if (C <= 4) SAIL_VARIANT(32, 4, 28, 1)
+        if (C <= 8) SAIL_VARIANT(32, 8, 16, 1)
+        SAIL_VARIANT(32, 16, 12, 1)
+    }
+    if (G == 32) {                                     // req == 33: software-pipelined form
+        if (C <= 4) SAIL_VARIANT(32, 4, 16, 0)
+        if (C <= 8) SAIL_VARIANT(32, 8, 12, 0)
+        SAIL_VARIANT(32, 16, 8, 0)
+    }
+    if (G == 16) {
+        if (C <= 4) SAIL_VARIANT(16, 4, 16, 0)
+        if (C <= 8) SAIL_VARIANT(16, 8, 12, 0)
+        SAIL_VARIANT(16, 16, 8, 0)
+    }
+    if (C <= 4) SAIL_VARIANT(8, 4, 16, 0)
+    if (C <= 8) SAIL_VARIANT(8, 8, 12, 0)
+    SAIL_VARIANT(8, 16, 8, 0)
 #undef SAIL_VARIANT
-    return set_err(h, SAIL_ERR_ARG, "no sweep kernel variant for lanes=%d, tau-points per lane=%d", G, C);
 }
 
 } // namespace sail
