@@ -765,6 +765,228 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
     }
 }
 
+// ---- several walkers per warp, screened: G lanes per walker, 32/G walkers per warp -----------------------------
+// The same moves and decisions as sweep_kernel_mask, with the instruction stream shared by the 32/G walkers of
+// a warp: one FP64 / shared-memory / shuffle instruction serves all of them, the reduction has log2(G) stages,
+// and tau-grids that are not a multiple of 32 waste fewer lanes (N_tau = 100: 8 x 13 = 104 slots instead of 128).
+// Each walker keeps its own cursor into a 32-move batch of staged proposals; a step screens the G-move window
+// that holds the cursor (one move per lane, ballot), takes the first feasible move of every walker, evaluates
+// Delta chi^2 for all walkers at once and applies the Metropolis decisions with predicated updates.  A walker
+// whose batch is exhausted idles (predicated off) until the others finish theirs.
+template <int G, int C, int MAXW, bool FACT, bool TRACE, bool W2REG>
+__global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kernel_sub(const SweepArgs P)
+{
+    constexpr int NW = 32 / G;
+    constexpr int LG = (G == 8) ? 3 : (G == 16) ? 4 : 5;
+    constexpr uint32_t GM = (G == 32) ? 0xffffffffu : ((1u << G) - 1u);
+    extern __shared__ __align__(16) unsigned char smem[];
+    double *s_ratio = reinterpret_cast<double *>(smem);
+    const int n_omega = P.n_omega;
+    const int n_omega_pad = (n_omega + 1) & ~1;
+    double *s_invd = s_ratio + n_omega_pad;
+    double *s_wm = s_invd + n_omega_pad;
+    double *s_E0 = s_wm + n_omega_pad;
+    const int e0_elems = FACT ? (P.n_hi + P.n_lo) * G : n_omega * G;
+    unsigned char *s_recs = reinterpret_cast<unsigned char *>(s_E0 + ((e0_elems + 1) & ~1));
+    for (int i = threadIdx.x; i < n_omega; i += blockDim.x) {
+        s_ratio[i] = P.ratio[i]; s_invd[i] = P.invd[i]; s_wm[i] = __dadd_rn(P.omega[i], 0.5 * P.domega);
+    }
+    for (int i = threadIdx.x; i < e0_elems; i += blockDim.x) s_E0[i] = P.E0[i];
+    // NW x 32 records per warp; slots beyond a short last batch are read (and masked out) by the screen
+    for (int i = threadIdx.x; i < (int)(blockDim.x * NW * (kRecMaskBytes / 4)); i += blockDim.x)
+        reinterpret_cast<uint32_t *>(s_recs)[i] = 0u;
+    __syncthreads();
+
+    const int lane = threadIdx.x & 31;
+    const int warp = threadIdx.x >> 5;
+    const int sub = lane % G;
+    const int q = lane / G;
+    // records of this lane's walker
+    uint32_t rbase = (uint32_t)__cvta_generic_to_shared(s_recs) + (uint32_t)((warp * NW + q) * 32 * kRecMaskBytes);
+    uint32_t e0_lane = (uint32_t)__cvta_generic_to_shared(s_E0) + (uint32_t)(sub * 8);
+    asm volatile("" : "+r"(rbase), "+r"(e0_lane));
+    unsigned char *const rec_gen = s_recs + (size_t)((warp * NW + q) * 32) * kRecMaskBytes;
+    const uint32_t e0_lo = e0_lane + (uint32_t)(P.n_hi * G * 8);
+    const int warps_per_cta = blockDim.x >> 5;
+    const int fshift = P.fact_shift;
+    const int fmask = (1 << fshift) - 1;
+    const int gshift = q * G;
+
+    for (long long grp = (long long)blockIdx.x * warps_per_cta + warp; grp < P.n_groups; grp += (long long)gridDim.x * warps_per_cta) {
+        const long long w = grp * NW + q;                          // < W_pad: always a valid slot
+        uint32_t wbase = (uint32_t)(w * n_omega);
+        asm volatile("" : "+r"(wbase));
+        double *const a_all = P.a;
+        double mt[C], G2[C], Wt[C], d[C], W2[W2REG ? C : 1];
+#pragma unroll
+        for (int i = 0; i < C; ++i) {
+            const int j = sub + G * i;
+            const bool ok = j < P.n_tau;
+            mt[i] = ok ? P.mt[(size_t)w * P.n_tau + j] : 0.0;
+            Wt[i] = ok ? P.Wj[j] : 0.0;
+            if (W2REG) W2[i] = Wt[i] + Wt[i];
+            d[i] = 0.0;
+        }
+        double chi2 = P.chi2[w];
+        double g = 1.0, ginv = 1.0;
+        bool tracing = false;
+        if (TRACE) tracing = P.trace != nullptr && w >= P.trace_lo && w < P.trace_hi;
+
+        for (int isw = 0; isw < P.n_sweeps; ++isw) {
+            int acc_sweep = 0, eval_sweep = 0;
+#pragma unroll
+            for (int i = 0; i < C; ++i) {
+                const int j = sub + G * i;
+                const double f = (j < P.n_tau) ? P.fj[j] : 0.0;
+                G2[i] = 2.0 * Wt[i] * (mt[i] - f);
+            }
+            const double y_sweep = P.y[w];
+            const double T_sweep = P.T[isw];
+            for (int m0 = 0; m0 < n_omega; m0 += 32) {
+                const int nb = min(32, n_omega - m0);
+                // ---- proposals (row A2): this walker's moves m0 .. m0+nb-1, G per pass ----------------------
+#pragma unroll 1
+                for (int k = sub; k < nb; k += G)
+                    propose_mask(P, (uint32_t)w, (uint32_t)(P.sweep0 + isw), (uint32_t)(m0 + k), y_sweep, T_sweep,
+                                 s_ratio, s_invd, s_wm, rec_gen + k * kRecMaskBytes);
+                __syncwarp();
+
+                int cur = 0;                           // next move of this walker's batch (uniform in the group)
+                while (true) {
+                    // ---- positivity screen (row A3) of the window that holds the cursor ----------------------
+                    int m = 0;
+                    double apn, asn;
+                    bool active;
+                    while (true) {
+                        active = cur < nb;
+                        const int base = active ? (cur & ~(G - 1)) : 0;
+                        const int idx = base + sub;
+                        const uint32_t rq = rbase + (uint32_t)(idx * kRecMaskBytes);
+                        const int4 q0 = lds_s32x4(rq);
+                        const double2 qd = lds_f64x2(rq + 16);
+                        const double a_p = ldg_f64(elem_ptr(a_all, wbase + (uint32_t)q0.x));
+                        const double a_s = ldg_f64(elem_ptr(a_all, wbase + (uint32_t)q0.y));
+                        const double qa = __hiloint2double(q0.w, q0.z);
+                        const double gn = fma(qa, g, g);
+                        apn = fma(gn, a_p, qd.x);
+                        asn = fma(gn, a_s, qd.y);
+                        const bool in_play = active && idx >= cur && idx < nb;
+                        const bool feas = in_play && ((__double2hiint(apn) | __double2hiint(asn)) >= 0);
+                        const uint32_t gb = (__ballot_sync(0xffffffffu, feas) >> gshift) & GM;
+                        const bool exhausted = active && gb == 0u;
+                        const int wend = min(base + G, nb);
+                        if (TRACE) {
+                            // moves of this window that are passed over as infeasible: [cur, m) or [cur, wend)
+                            const int upto = exhausted ? wend : (gb ? base + __ffs((int)gb) - 1 : cur);
+                            if (active && idx >= cur && idx < upto && w < P.W) {
+                                const double2 qt = lds_f64x2(rq + 64);
+                                const size_t mv = ((size_t)(P.call_off + isw)) * n_omega + m0 + idx;
+                                if (P.flags) P.flags[(size_t)w * P.call_sweeps * n_omega + mv] = (uint8_t)0;
+                                if (tracing) {
+                                    sail_trace_rec *tr = P.trace + ((size_t)(w - P.trace_lo) * P.call_sweeps * n_omega + mv);
+                                    tr->p = q0.x; tr->s = q0.y; tr->flags = 0; tr->move = m0 + idx;
+                                    tr->rho = 1.0 + qa; tr->delta_p = qd.x; tr->delta_s = qd.y;
+                                    tr->dchi2 = 0.0; tr->thr = qt.x; tr->ap_new = apn; tr->as_new = asn;
+                                }
+                            }
+                        }
+                        if (exhausted) cur = wend;
+                        else if (gb) m = base + __ffs((int)gb) - 1;
+                        if (!__any_sync(0xffffffffu, exhausted && cur < nb)) { active = cur < nb; break; }
+                    }
+                    if (!__any_sync(0xffffffffu, active)) break;
+
+                    // ---- incremental Delta chi^2 over all tau (row A4) for the move m of every walker ----------
+                    const uint32_t r = rbase + (uint32_t)(m * kRecMaskBytes);
+                    const int4 r0 = lds_s32x4(r);
+                    const double2 dd = lds_f64x2(r + 16);
+                    const double2 dr = lds_f64x2(r + 32);
+                    const double2 sc = lds_f64x2(r + 48);
+                    const double2 th = lds_f64x2(r + 64);
+                    const double alpha = __hiloint2double(r0.w, r0.z);
+                    double e0p, e0s;
+                    if (FACT) {
+                        e0p = lds_f64(e0_lane + (uint32_t)((r0.x >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.x & fmask) * (G * 8)));
+                        e0s = lds_f64(e0_lane + (uint32_t)((r0.y >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.y & fmask) * (G * 8)));
+                    } else {
+                        e0p = lds_f64(e0_lane + (uint32_t)(r0.x * (G * 8)));
+                        e0s = lds_f64(e0_lane + (uint32_t)(r0.y * (G * 8)));
+                    }
+                    double vm = fma(dd.x, e0p, dd.y * e0s);
+                    double vc = fma(dr.x, e0p, dr.y * e0s);
+                    double acc_a = 0.0, acc_b = 0.0;
+#pragma unroll
+                    for (int i = 0; i < C; ++i) {
+                        double vi;
+                        if (i == 0) vi = vm;
+                        else if (i == 1) vi = vc;
+                        else { vi = fma(sc.x, vc, sc.y * vm); vm = vc; vc = vi; }
+                        d[i] = fma(alpha, mt[i], vi);
+                        const double t = fma(Wt[i], d[i], G2[i]);
+                        if (i & 1) acc_b = fma(d[i], t, acc_b);
+                        else       acc_a = fma(d[i], t, acc_a);
+                    }
+                    double dchi2 = (C > 1) ? acc_a + acc_b : acc_a;
+#pragma unroll
+                    for (int off = G / 2; off > 0; off >>= 1) dchi2 += __shfl_xor_sync(0xffffffffu, dchi2, off);
+                    // ---- Metropolis (row A5, Eq. 10), per walker; updates are predicated, not branched --------
+                    const bool acc = active && (dchi2 < th.x);
+                    const int ia = acc ? 1 : 0;
+                    if (__any_sync(0xffffffffu, acc)) {
+#pragma unroll
+                        for (int i = 0; i < C; ++i) {
+                            add_if(mt[i], d[i], ia);
+                            if (W2REG) fma_if(G2[i], W2[i], d[i], ia);
+                            else       fma_if(G2[i], Wt[i], d[i] + d[i], ia);
+                        }
+                        add_if(chi2, dchi2, ia);
+                        fma_if(g, alpha, g, ia);
+                        mul_if(ginv, th.y, ia);
+                        const int mine = (acc && sub == (m & (G - 1))) ? 1 : 0;
+                        stg_f64_if(elem_ptr(a_all, wbase + (uint32_t)r0.x), apn * ginv, mine);
+                        stg_f64_if(elem_ptr(a_all, wbase + (uint32_t)r0.y), asn * ginv, mine);
+                        acc_sweep += ia;
+                    }
+                    eval_sweep += active ? 1 : 0;
+                    if (TRACE) {
+                        if (active && sub == (m & (G - 1)) && w < P.W) {
+                            const int fl = 5 | (ia << 1);
+                            const size_t mv = ((size_t)(P.call_off + isw)) * n_omega + m0 + m;
+                            if (P.flags) P.flags[(size_t)w * P.call_sweeps * n_omega + mv] = (uint8_t)fl;
+                            if (tracing) {
+                                sail_trace_rec *tr = P.trace + ((size_t)(w - P.trace_lo) * P.call_sweeps * n_omega + mv);
+                                tr->p = r0.x; tr->s = r0.y; tr->flags = fl; tr->move = m0 + m;
+                                tr->rho = 1.0 + alpha; tr->delta_p = dd.x; tr->delta_s = dd.y;
+                                tr->dchi2 = dchi2; tr->thr = th.x; tr->ap_new = apn; tr->as_new = asn;
+                            }
+                        }
+                    }
+                    if (active) cur = m + 1;
+                    __syncwarp();
+                }
+                __syncwarp();
+            }
+            // ---- end of sweep: fold the lazy scale (Eq. 19), counters, y (row A6, Eq. 30) ----------------
+            for (int k = sub; k < n_omega; k += G) a_all[(size_t)wbase + k] *= g;
+            g = 1.0;
+            ginv = 1.0;
+            if (sub == 0) {
+                P.n_acc[w] += (unsigned long long)acc_sweep;
+                P.n_eval[w] += (unsigned long long)eval_sweep;
+                P.y[w] = amp_factor(P, acc_sweep, y_sweep);
+            }
+            __syncwarp();
+        }
+#pragma unroll
+        for (int i = 0; i < C; ++i) {
+            const int j = sub + G * i;
+            if (j < P.n_tau) P.mt[(size_t)w * P.n_tau + j] = mt[i];
+        }
+        if (sub == 0) P.chi2[w] = chi2;
+        __syncwarp();
+    }
+}
+
 // ---- sweep tables: ratio[k] = exp(-omega_k G dtau); invd[k] = 1/(k domega); start values E0 ----------
 __global__ void sweep_tables_kernel(int n_omega, int G, double domega, double tau0, double dtau,
                                     const double *omega, int fact, int shift, int n_hi, int n_lo,
@@ -825,12 +1047,13 @@ int ensure_sweep_tables(sail_handle *h, int G)
 
 // ---- dispatch -----------------------------------------------------------------------------------------
 // MODE 0: sub-warp groups / software pipeline (sweep_kernel), 1: lean one walker per warp (sweep_kernel_warp),
-//      2: screened one walker per warp (sweep_kernel_mask), 3: the same with 2 Wj in registers
+//      2: screened one walker per warp (sweep_kernel_mask), 3: the same with 2 Wj in registers,
+//      4: screened sub-warp groups (sweep_kernel_sub), 5: the same with 2 Wj in registers
 template <int G, int C, int MAXW, bool FACT, bool TRACE, int MODE = 0>
 static int launch_variant(sail_handle *h, SweepArgs &args)
 {
     constexpr int NW = 32 / G;
-    constexpr int rec_bytes = (MODE >= 2) ? kRecMaskBytes : kRecBytes;
+    constexpr int rec_bytes = (MODE >= 4) ? NW * kRecMaskBytes : (MODE >= 2) ? kRecMaskBytes : kRecBytes;
     args.n_groups = (args.W + NW - 1) / NW;
     int warps = (int)((args.n_groups + h->num_sms - 1) / h->num_sms);
     if (warps > MAXW) warps = MAXW;
@@ -843,7 +1066,9 @@ static int launch_variant(sail_handle *h, SweepArgs &args)
     if (smem > 227 * 1024)
         return set_err(h, SAIL_ERR_ARG, "sweep tables need %zu bytes of shared memory (> 227 KB)", smem);
     void (*kern)(const SweepArgs);
-    if constexpr (MODE == 3) kern = sweep_kernel_mask<C, MAXW, FACT, TRACE, true>;
+    if constexpr (MODE == 5) kern = sweep_kernel_sub<G, C, MAXW, FACT, TRACE, true>;
+    else if constexpr (MODE == 4) kern = sweep_kernel_sub<G, C, MAXW, FACT, TRACE, false>;
+    else if constexpr (MODE == 3) kern = sweep_kernel_mask<C, MAXW, FACT, TRACE, true>;
     else if constexpr (MODE == 2) kern = sweep_kernel_mask<C, MAXW, FACT, TRACE, false>;
     else if constexpr (MODE == 1) kern = sweep_kernel_warp<C, MAXW, FACT, TRACE>;
     else kern = sweep_kernel<G, C, MAXW, FACT, TRACE>;
@@ -928,13 +1153,16 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
         SAIL_VARIANT(32, 16, 8, 0)
     }
     if (G == 16) {
-        if (C <= 4) SAIL_VARIANT(16, 4, 16, 0)
-        if (C <= 8) SAIL_VARIANT(16, 8, 12, 0)
-        SAIL_VARIANT(16, 16, 8, 0)
+        if (C <= 4) SAIL_VARIANT(16, 4, 16, 5)
+        if (C <= 7) SAIL_VARIANT(16, 7, 16, 5)
+        if (C <= 8) SAIL_VARIANT(16, 8, 16, 5)
+        if (C <= 13) SAIL_VARIANT(16, 13, 8, 5)
+        SAIL_VARIANT(16, 16, 8, 5)
     }
-    if (C <= 4) SAIL_VARIANT(8, 4, 16, 0)
-    if (C <= 8) SAIL_VARIANT(8, 8, 12, 0)
-    SAIL_VARIANT(8, 16, 8, 0)
+    if (C <= 4) SAIL_VARIANT(8, 4, 16, 5)
+    if (C <= 8) SAIL_VARIANT(8, 8, 12, 5)
+    if (C <= 13) SAIL_VARIANT(8, 13, 8, 5)
+    SAIL_VARIANT(8, 16, 8, 5)
 #undef SAIL_VARIANT
 }
 
