@@ -20,9 +20,11 @@ _LIB = os.path.join(_HERE, "libsail_oracle.so")
 def build(force: bool = False) -> str:
     """Compile the oracle with gcc (strict IEEE: no FMA contraction, no fast-math)."""
     if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        tmp = f"{_LIB}.{os.getpid()}.tmp"      # atomic: concurrent processes (gloo tests) never see a partial file
         cmd = ["gcc", "-O2", "-std=c11", "-ffp-contract=off", "-fno-fast-math", "-fopenmp", "-fPIC",
-               "-shared", "-o", _LIB, _SRC, "-lm"]
+               "-shared", "-o", tmp, _SRC, "-lm"]
         subprocess.run(cmd, check=True)
+        os.replace(tmp, _LIB)
     return _LIB
 
 
