@@ -18,93 +18,9 @@
 // into a~ at the end of every sweep.
 // Walker slots W .. W_pad-1 (W_pad = W rounded up to 4) are scratch copies of the last walker so that a
 // warp never has an inactive group: no activity predicate in the hot loop; they are never reported.
-#include "sail_internal.cuh"
+#include "sweep_common.cuh"
 
 namespace sail {
-
-struct SweepArgs {
-    int n_omega, n_tau;
-    long long W, n_groups;
-    double A, B, omega_mid0, domega, eta, amp_p, amp_m, y_min;
-    int amp_mode;
-    uint32_t seed_lo, seed_hi;
-    const double *Wj, *fj, *ratio, *E0, *invd, *omega;
-    int fact, fact_shift, n_hi, n_lo;
-    double *a, *mt, *chi2, *y;
-    unsigned long long *n_acc, *n_eval;
-    const double *T;
-    long long sweep0;
-    int n_sweeps;
-    long long trace_lo, trace_hi;
-    sail_trace_rec *trace;
-    uint8_t *flags;
-    long long call_sweeps, call_off;   // sweeps in the whole sail_anneal call / offset of this launch
-};
-
-// 1/x for x close to 1 (|x - 1| < 0.5): hardware seed + two Newton steps, relative error ~1e-16.
-__device__ __forceinline__ double fast_recip(double x)
-{
-    double r;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(r) : "d"(x));
-    double e = fma(-x, r, 1.0);
-    r = fma(r, e, r);
-    e = fma(-x, r, 1.0);
-    return fma(r, e, r);
-}
-
-// shared-memory accesses by 32-bit shared-window address (no generic-address arithmetic in the hot loop)
-__device__ __forceinline__ double lds_f64(uint32_t addr)
-{
-    double v;
-    asm volatile("ld.shared.f64 %0, [%1];" : "=d"(v) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ double2 lds_f64x2(uint32_t addr)
-{
-    double2 v;
-    asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(addr));
-    return v;
-}
-__device__ __forceinline__ int4 lds_s32x4(uint32_t addr)
-{
-    int4 v;
-    asm volatile("ld.shared.v4.s32 {%0, %1, %2, %3}, [%4];" : "=r"(v.x), "=r"(v.y), "=r"(v.z), "=r"(v.w) : "r"(addr));
-    return v;
-}
-
-// element pointer a + idx (idx < 2^32) in one IMAD.WIDE
-__device__ __forceinline__ double *elem_ptr(double *base, uint32_t idx)
-{
-    unsigned long long r;
-    asm("mad.wide.u32 %0, %1, 8, %2;" : "=l"(r) : "r"(idx), "l"(reinterpret_cast<unsigned long long>(base)));
-    return reinterpret_cast<double *>(r);
-}
-__device__ __forceinline__ double ldg_f64(const double *p)
-{
-    double v;
-    asm volatile("ld.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
-    return v;
-}
-// predicated (not branched) store: only the lanes with pred != 0 write
-__device__ __forceinline__ void stg_f64_if(double *p, double v, int pred)
-{
-    asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %2, 0;\n\t@q st.global.f64 [%0], %1;\n\t}" :: "l"(p), "d"(v), "r"(pred) : "memory");
-}
-// predicated (not branched) FP64 updates: lanes of walkers that did not accept keep their state without
-// the warp diverging
-__device__ __forceinline__ void add_if(double &x, double y, int pred)
-{
-    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %2, 0;\n\t@p add.rn.f64 %0, %0, %1;\n\t}" : "+d"(x) : "d"(y), "r"(pred));
-}
-__device__ __forceinline__ void fma_if(double &x, double a, double b, int pred)
-{
-    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %3, 0;\n\t@p fma.rn.f64 %0, %1, %2, %0;\n\t}" : "+d"(x) : "d"(a), "d"(b), "r"(pred));
-}
-__device__ __forceinline__ void mul_if(double &x, double a, int pred)
-{
-    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %2, 0;\n\t@p mul.rn.f64 %0, %0, %1;\n\t}" : "+d"(x) : "d"(a), "r"(pred));
-}
-
 
 // ---- one proposal (row A2): Philox4x32-10 keyed by (seed; walker, sweep, move, 0) -> 64-byte record ------
 //   [ 0] p, s (int32), alpha = rho - 1      [16] delta_p, delta_s (Eq. 20-21)
@@ -135,234 +51,6 @@ __device__ __forceinline__ void propose(const SweepArgs &P, uint32_t walker, uin
     *reinterpret_cast<double2 *>(rec + 32) = make_double2(thr, fast_recip(rho));
     *reinterpret_cast<double2 *>(rec + 48) = make_double2(s_ratio[p], s_ratio[s]);
 }
-
-// Eq. 30: y from the sweep's acceptance rate
-__device__ __forceinline__ double amp_factor(const SweepArgs &P, int acc_sweep, double y)
-{
-    if (P.amp_mode != 1) return y;
-    const double rate = (double)acc_sweep / (double)P.n_omega;
-    if (rate >= P.amp_p) return 1.0;
-    const double x = rate / P.amp_p;
-    const double yy = (P.amp_m == 2.0) ? x * x : pow(x, P.amp_m);
-    return yy < P.y_min ? P.y_min : yy;
-}
-
-// MAXW = warps per CTA (one CTA per SM) the variant is register-budgeted for; the register file is allocated in
-// units of 4 warps per CTA, so the budget is 65536 / (roundup4(MAXW) * 32) registers per thread.
-// FACT: start values E0[k][l] = H[k_hi][l] * L[k_lo][l] (two small tables) instead of one N_omega x G table.
-template <int G, int C, int MAXW, bool FACT, bool TRACE>
-__global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kernel(const SweepArgs P)
-{
-    constexpr int NW = 32 / G;               // walkers per warp
-    extern __shared__ __align__(16) unsigned char smem[];
-    double *s_ratio = reinterpret_cast<double *>(smem);
-    const int n_omega = P.n_omega;
-    const int n_omega_pad = (n_omega + 1) & ~1;
-    double *s_invd = s_ratio + n_omega_pad;                       // 1 / (k domega), k = 1 .. n_omega-1
-    double *s_wm = s_invd + n_omega_pad;                          // bin midpoints omega_k + domega/2
-    double *s_E0 = s_wm + n_omega_pad;
-    const int e0_elems = FACT ? (P.n_hi + P.n_lo) * G : n_omega * G;
-    unsigned char *s_recs = reinterpret_cast<unsigned char *>(s_E0 + ((e0_elems + 1) & ~1));
-
-    for (int i = threadIdx.x; i < n_omega; i += blockDim.x) {
-        s_ratio[i] = P.ratio[i]; s_invd[i] = P.invd[i]; s_wm[i] = __dadd_rn(P.omega[i], 0.5 * P.domega);
-    }
-    for (int i = threadIdx.x; i < e0_elems; i += blockDim.x) s_E0[i] = P.E0[i];
-    __syncthreads();
-
-    const int lane = threadIdx.x & 31;
-    const int warp = threadIdx.x >> 5;
-    const int sub = lane % G;                // lane within the walker's group
-    const int q = lane / G;                  // which walker of the warp
-    unsigned char *my_rec_w = s_recs + ((size_t)warp * 32 + lane) * kRecBytes;       // record this lane writes
-    // 32-bit shared addresses: records this lane's group reads, this lane's column of the start table(s)
-    const uint32_t rbase = (uint32_t)__cvta_generic_to_shared(s_recs) + (uint32_t)((warp * 32 + q * G) * kRecBytes);
-    const uint32_t e0_lane = (uint32_t)__cvta_generic_to_shared(s_E0) + (uint32_t)(sub * 8);
-    const uint32_t e0_lo = e0_lane + (uint32_t)(P.n_hi * G * 8);                     // FACT: low-part table
-    const int warps_per_cta = blockDim.x >> 5;
-    const long long total_warps = (long long)gridDim.x * warps_per_cta;
-    const int fshift = P.fact_shift;
-    const int fmask = (1 << fshift) - 1;
-    const bool leader = (sub == 0);
-
-    for (long long grp = (long long)blockIdx.x * warps_per_cta + warp; grp < P.n_groups; grp += total_warps) {
-        const long long w = grp * NW + q;                          // < W_pad: always a valid slot
-        double *__restrict__ a_w = P.a + (size_t)w * n_omega;
-
-        // ---- load the walker's residual state into registers --------------------------------------
-        double mt[C], G2[C], Wt[C], d[C], v[C];
-#pragma unroll
-        for (int i = 0; i < C; ++i) {
-            const int j = sub + G * i;
-            const bool ok = j < P.n_tau;
-            mt[i] = ok ? P.mt[(size_t)w * P.n_tau + j] : 0.0;
-            Wt[i] = ok ? P.Wj[j] : 0.0;
-            d[i] = 0.0;
-            v[i] = 0.0;
-        }
-        double chi2 = P.chi2[w];
-        double y = P.y[w];
-        double g = 1.0, ginv = 1.0;
-        bool tracing = false;
-        if (TRACE) tracing = P.trace != nullptr && w >= P.trace_lo && w < P.trace_hi;
-
-        for (int isw = 0; isw < P.n_sweeps; ++isw) {
-            const uint32_t sweep = (uint32_t)(P.sweep0 + isw);
-            int acc_sweep = 0, eval_sweep = 0;
-            // G2 is a pure function of mt at every sweep start, so splitting a run into several calls
-            // (state round-trips through global memory) reproduces the single-call chain bit for bit
-#pragma unroll
-            for (int i = 0; i < C; ++i) {
-                const int j = sub + G * i;
-                const double f = (j < P.n_tau) ? P.fj[j] : 0.0;
-                G2[i] = 2.0 * Wt[i] * (mt[i] - f);
-            }
-
-            for (int m0 = 0; m0 < n_omega; m0 += G) {
-                const int nb = min(G, n_omega - m0);
-                // ---- proposals for moves m0 .. m0+nb-1, one per lane (row A2) -----------------------
-                if (sub < nb)
-                    propose(P, (uint32_t)w, sweep, (uint32_t)(m0 + sub), y, P.T[isw], s_ratio, s_invd, s_wm, my_rec_w);
-                __syncwarp();
-
-                // ---- software pipeline -------------------------------------------------------------------
-                // Everything of move mm+1 that does not depend on the chain state (record, start values,
-                // v_i = delta_p E_p,i + delta_s E_s,i by the geometric recurrence, the two spectrum
-                // coefficients) is prepared while move mm's reduction is in flight.
-                int4 r0;            // p, s, alpha
-                double2 dd, th;     // (delta_p, delta_s), (threshold, 1/rho)
-                double ap_t, as_t;  // a~_p, a~_s (patched if move mm rewrites them)
-                auto prepare = [&](int mm) {
-                    const uint32_t r = rbase + (uint32_t)(mm * kRecBytes);
-                    r0 = lds_s32x4(r);
-                    dd = lds_f64x2(r + 16);
-                    th = lds_f64x2(r + 32);
-                    const double2 rr = lds_f64x2(r + 48);
-                    ap_t = ldg_f64(elem_ptr(a_w, (uint32_t)r0.x));
-                    as_t = ldg_f64(elem_ptr(a_w, (uint32_t)r0.y));
-                    double e0p, e0s;
-                    if (FACT) {
-                        e0p = lds_f64(e0_lane + (uint32_t)((r0.x >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.x & fmask) * (G * 8)));
-                        e0s = lds_f64(e0_lane + (uint32_t)((r0.y >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.y & fmask) * (G * 8)));
-                    } else {
-                        e0p = lds_f64(e0_lane + (uint32_t)(r0.x * (G * 8)));
-                        e0s = lds_f64(e0_lane + (uint32_t)(r0.y * (G * 8)));
-                    }
-                    // geometric recurrence, two interleaved sub-chains per row (even / odd i) to halve its depth
-                    double ep0 = dd.x * e0p, es0 = dd.y * e0s;
-                    double ep1 = ep0 * rr.x, es1 = es0 * rr.y;
-                    const double rp2 = rr.x * rr.x, rs2 = rr.y * rr.y;
-#pragma unroll
-                    for (int i = 0; i < C; i += 2) {
-                        v[i] = ep0 + es0;
-                        if (i + 1 < C) v[i + 1] = ep1 + es1;
-                        if (i + 2 < C) { ep0 *= rp2; es0 *= rs2; }
-                        if (i + 3 < C) { ep1 *= rp2; es1 *= rs2; }
-                    }
-                };
-                prepare(0);
-
-                for (int mm = 0; mm < nb; ++mm) {
-                    const int p = r0.x, s = r0.y;
-                    const double alpha = __hiloint2double(r0.w, r0.z);
-                    const double dpv = dd.x, dsv = dd.y, thr = th.x, inv_rho = th.y;
-                    // ---- positivity (row A3): sign bits of rho a_p + delta_p, rho a_s + delta_s
-                    const double gn = fma(alpha, g, g);                 // rho * g, exactly rounded
-                    const double ap_new = fma(gn, ap_t, dpv);
-                    const double as_new = fma(gn, as_t, dsv);
-                    const bool feas = (__double2hiint(ap_new) | __double2hiint(as_new)) >= 0;
-                    // one walker per warp: an infeasible move skips the tau loop (warp-uniform branch);
-                    // several walkers per warp: always evaluate, infeasible groups just cannot accept
-                    const bool do_eval = (G == 32) ? feas : true;
-                    // ---- incremental Delta chi^2 over all tau (row A4, Eq. 22 + Eq. 9) -------------------
-                    double dchi2 = 0.0;
-                    if (do_eval) {
-                        double acc_a = 0.0, acc_b = 0.0;
-#pragma unroll
-                        for (int i = 0; i < C; ++i) {
-                            d[i] = fma(alpha, mt[i], v[i]);
-                            const double t = fma(Wt[i], d[i], G2[i]);
-                            if (i & 1) acc_b = fma(d[i], t, acc_b);
-                            else       acc_a = fma(d[i], t, acc_a);
-                        }
-                        dchi2 = (C > 1) ? acc_a + acc_b : acc_a;
-                    }
-                    // prepare the next move (clamped: the last step re-prepares
-                    // itself, harmlessly) — no branch, so the scheduler can interleave it with the reduction below
-                    prepare(min(mm + 1, nb - 1));
-                    int fl = feas ? 1 : 0;
-                    if (do_eval) {
-#pragma unroll
-                        for (int off = G / 2; off > 0; off >>= 1) dchi2 += __shfl_xor_sync(0xffffffffu, dchi2, off);
-                        fl |= 4;
-                        // ---- Metropolis (row A5, Eq. 10): accept iff dchi2/T + ln u < 0 ------------------
-                        const bool acc = feas && (dchi2 < thr);
-                        if (__any_sync(0xffffffffu, acc)) {
-                            const int ia = acc ? 1 : 0;
-#pragma unroll
-                            for (int i = 0; i < C; ++i) {
-                                add_if(mt[i], d[i], ia);
-                                fma_if(G2[i], Wt[i], d[i] + d[i], ia);
-                            }
-                            add_if(chi2, dchi2, ia);
-                            g = acc ? gn : g;
-                            mul_if(ginv, inv_rho, ia);
-                            const double ap_store = ap_new * ginv, as_store = as_new * ginv;
-                            stg_f64_if(elem_ptr(a_w, (uint32_t)p), ap_store, (leader && acc) ? 1 : 0);
-                            stg_f64_if(elem_ptr(a_w, (uint32_t)s), as_store, (leader && acc) ? 1 : 0);
-                            // the next move's coefficients were fetched before this store
-                            if (acc) {
-                                if (r0.x == p) ap_t = ap_store; else if (r0.x == s) ap_t = as_store;
-                                if (r0.y == p) as_t = ap_store; else if (r0.y == s) as_t = as_store;
-                            }
-                            acc_sweep += ia;
-                            fl |= ia << 1;
-                            __syncwarp();
-                        }
-                    }
-                    eval_sweep += fl & 1;
-                    if (TRACE) {
-                        if (leader && w < P.W) {
-                            const size_t mv = ((size_t)(P.call_off + isw)) * n_omega + m0 + mm;
-                            if (P.flags) P.flags[(size_t)w * P.call_sweeps * n_omega + mv] = (uint8_t)fl;
-                            if (tracing) {
-                                sail_trace_rec *tr = P.trace + ((size_t)(w - P.trace_lo) * P.call_sweeps * n_omega + mv);
-                                tr->p = p; tr->s = s; tr->flags = fl; tr->move = m0 + mm;
-                                tr->rho = 1.0 + alpha; tr->delta_p = dpv; tr->delta_s = dsv;
-                                tr->dchi2 = dchi2; tr->thr = thr; tr->ap_new = ap_new; tr->as_new = as_new;
-                            }
-                        }
-                    }
-                }
-                __syncwarp();
-            }
-
-            // ---- end of sweep: fold the lazy scale (Eq. 19), counters, y (row A6, Eq. 30) ------------
-            for (int k = sub; k < n_omega; k += G) a_w[k] *= g;
-            g = 1.0;
-            ginv = 1.0;
-            if (leader) {
-                P.n_acc[w] += (unsigned long long)acc_sweep;
-                P.n_eval[w] += (unsigned long long)eval_sweep;
-            }
-            y = amp_factor(P, acc_sweep, y);
-            __syncwarp();
-        }
-
-        // ---- store the state back ----------------------------------------------------------------
-#pragma unroll
-        for (int i = 0; i < C; ++i) {
-            const int j = sub + G * i;
-            if (j < P.n_tau) P.mt[(size_t)w * P.n_tau + j] = mt[i];
-        }
-        if (leader) {
-            P.chi2[w] = chi2;
-            P.y[w] = y;
-        }
-        __syncwarp();
-    }
-}
-
 
 // ---- one walker per WARP, register-lean (<= 72 registers: 28 resident warps per SM = 7 per sub-partition) ------
 // Same arithmetic as sweep_kernel<32, C, ...>; no software pipeline (the other six warps of the sub-partition hide
@@ -546,36 +234,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
 //    and propagate through the bounded Green's function (r_p^{n+1} - r_s^{n+1})/(r_p - r_s) <= n + 1.
 //  * with W2REG the constants 2 Wj live in registers as well: the accepted update is 2 instructions per
 //    tau-point instead of 3.
-constexpr int kRecMaskBytes = 80;
-// record: [0] p, s (int32), alpha = rho - 1   [16] delta_p, delta_s   [32] delta_p r_p, delta_s r_s
-//         [48] r_p + r_s, -(r_p r_s)          [64] thr = -T ln u_acc, 1/rho
-__device__ __forceinline__ void propose_mask(const SweepArgs &P, uint32_t walker, uint32_t sweep, uint32_t move, double y, double T,
-                                             const double *s_ratio, const double *s_invd, const double *s_wm, unsigned char *rec)
-{
-    uint32_t x[4];
-    philox4x32_10(walker, sweep, move, 0u, P.seed_lo, P.seed_hi, x);
-    const int p = (int)__umulhi(x[0], (uint32_t)P.n_omega);
-    int s = (int)__umulhi(x[1], (uint32_t)(P.n_omega - 1));
-    s += (s >= p) ? 1 : 0;
-    const double u_rho = ((double)x[2] + 0.5) * 2.3283064365386962890625e-10;
-    const double u_acc = ((double)x[3] + 0.5) * 2.3283064365386962890625e-10;
-    const double rho = __dsub_rn(1.0, __dmul_rn(__dmul_rn(y, P.eta), __dsub_rn(__dmul_rn(2.0, u_rho), 1.0)));
-    const double alpha = __dsub_rn(rho, 1.0);
-    const double omr = __dsub_rn(1.0, rho);
-    const int dps = p - s;
-    const double inv = (dps > 0) ? s_invd[dps] : -s_invd[-dps];
-    const double dp = __dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[s]))), inv);
-    const double ds = -__dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[p]))), inv);
-    const double thr = -T * log(u_acc);
-    const double rp = s_ratio[p], rs = s_ratio[s];
-    *reinterpret_cast<int4 *>(rec) = make_int4(p, s, __double2loint(alpha), __double2hiint(alpha));
-    *reinterpret_cast<double2 *>(rec + 16) = make_double2(dp, ds);
-    *reinterpret_cast<double2 *>(rec + 32) = make_double2(dp * rp, ds * rs);
-    *reinterpret_cast<double2 *>(rec + 48) = make_double2(rp + rs, -(rp * rs));
-    *reinterpret_cast<double2 *>(rec + 64) = make_double2(thr, fast_recip(rho));
-}
-
-template <int C, int MAXW, bool FACT, bool TRACE, bool W2REG>
+template <int C, int MAXW, bool FACT, bool TRACE, bool W2REG, bool DMMA>
 __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kernel_mask(const SweepArgs P)
 {
     constexpr int G = 32;
@@ -698,8 +357,12 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                         else       acc_a = fma(d[i], t, acc_a);
                     }
                     double dchi2 = (C > 1) ? acc_a + acc_b : acc_a;
+                    if (DMMA) {
+                        dchi2 = warp_sum_dmma(dchi2);
+                    } else {
 #pragma unroll
-                    for (int off = 16; off > 0; off >>= 1) dchi2 += __shfl_xor_sync(0xffffffffu, dchi2, off);
+                        for (int off = 16; off > 0; off >>= 1) dchi2 += __shfl_xor_sync(0xffffffffu, dchi2, off);
+                    }
                     eval_sweep++;
                     if (TRACE) { tr_eval |= 1u << m; if (lane == m) tr_dchi2 = dchi2; }
                     // ---- Metropolis (row A5, Eq. 10); identical in every lane: a uniform branch ----------
@@ -765,228 +428,6 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
     }
 }
 
-// ---- several walkers per warp, screened: G lanes per walker, 32/G walkers per warp -----------------------------
-// The same moves and decisions as sweep_kernel_mask, with the instruction stream shared by the 32/G walkers of
-// a warp: one FP64 / shared-memory / shuffle instruction serves all of them, the reduction has log2(G) stages,
-// and tau-grids that are not a multiple of 32 waste fewer lanes (N_tau = 100: 8 x 13 = 104 slots instead of 128).
-// Each walker keeps its own cursor into a 32-move batch of staged proposals; a step screens the G-move window
-// that holds the cursor (one move per lane, ballot), takes the first feasible move of every walker, evaluates
-// Delta chi^2 for all walkers at once and applies the Metropolis decisions with predicated updates.  A walker
-// whose batch is exhausted idles (predicated off) until the others finish theirs.
-template <int G, int C, int MAXW, bool FACT, bool TRACE, bool W2REG>
-__global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kernel_sub(const SweepArgs P)
-{
-    constexpr int NW = 32 / G;
-    constexpr int LG = (G == 8) ? 3 : (G == 16) ? 4 : 5;
-    constexpr uint32_t GM = (G == 32) ? 0xffffffffu : ((1u << G) - 1u);
-    extern __shared__ __align__(16) unsigned char smem[];
-    double *s_ratio = reinterpret_cast<double *>(smem);
-    const int n_omega = P.n_omega;
-    const int n_omega_pad = (n_omega + 1) & ~1;
-    double *s_invd = s_ratio + n_omega_pad;
-    double *s_wm = s_invd + n_omega_pad;
-    double *s_E0 = s_wm + n_omega_pad;
-    const int e0_elems = FACT ? (P.n_hi + P.n_lo) * G : n_omega * G;
-    unsigned char *s_recs = reinterpret_cast<unsigned char *>(s_E0 + ((e0_elems + 1) & ~1));
-    for (int i = threadIdx.x; i < n_omega; i += blockDim.x) {
-        s_ratio[i] = P.ratio[i]; s_invd[i] = P.invd[i]; s_wm[i] = __dadd_rn(P.omega[i], 0.5 * P.domega);
-    }
-    for (int i = threadIdx.x; i < e0_elems; i += blockDim.x) s_E0[i] = P.E0[i];
-    // NW x 32 records per warp; slots beyond a short last batch are read (and masked out) by the screen
-    for (int i = threadIdx.x; i < (int)(blockDim.x * NW * (kRecMaskBytes / 4)); i += blockDim.x)
-        reinterpret_cast<uint32_t *>(s_recs)[i] = 0u;
-    __syncthreads();
-
-    const int lane = threadIdx.x & 31;
-    const int warp = threadIdx.x >> 5;
-    const int sub = lane % G;
-    const int q = lane / G;
-    // records of this lane's walker
-    uint32_t rbase = (uint32_t)__cvta_generic_to_shared(s_recs) + (uint32_t)((warp * NW + q) * 32 * kRecMaskBytes);
-    uint32_t e0_lane = (uint32_t)__cvta_generic_to_shared(s_E0) + (uint32_t)(sub * 8);
-    asm volatile("" : "+r"(rbase), "+r"(e0_lane));
-    unsigned char *const rec_gen = s_recs + (size_t)((warp * NW + q) * 32) * kRecMaskBytes;
-    const uint32_t e0_lo = e0_lane + (uint32_t)(P.n_hi * G * 8);
-    const int warps_per_cta = blockDim.x >> 5;
-    const int fshift = P.fact_shift;
-    const int fmask = (1 << fshift) - 1;
-    const int gshift = q * G;
-
-    for (long long grp = (long long)blockIdx.x * warps_per_cta + warp; grp < P.n_groups; grp += (long long)gridDim.x * warps_per_cta) {
-        const long long w = grp * NW + q;                          // < W_pad: always a valid slot
-        uint32_t wbase = (uint32_t)(w * n_omega);
-        asm volatile("" : "+r"(wbase));
-        double *const a_all = P.a;
-        double mt[C], G2[C], Wt[C], d[C], W2[W2REG ? C : 1];
-#pragma unroll
-        for (int i = 0; i < C; ++i) {
-            const int j = sub + G * i;
-            const bool ok = j < P.n_tau;
-            mt[i] = ok ? P.mt[(size_t)w * P.n_tau + j] : 0.0;
-            Wt[i] = ok ? P.Wj[j] : 0.0;
-            if (W2REG) W2[i] = Wt[i] + Wt[i];
-            d[i] = 0.0;
-        }
-        double chi2 = P.chi2[w];
-        double g = 1.0, ginv = 1.0;
-        bool tracing = false;
-        if (TRACE) tracing = P.trace != nullptr && w >= P.trace_lo && w < P.trace_hi;
-
-        for (int isw = 0; isw < P.n_sweeps; ++isw) {
-            int acc_sweep = 0, eval_sweep = 0;
-#pragma unroll
-            for (int i = 0; i < C; ++i) {
-                const int j = sub + G * i;
-                const double f = (j < P.n_tau) ? P.fj[j] : 0.0;
-                G2[i] = 2.0 * Wt[i] * (mt[i] - f);
-            }
-            const double y_sweep = P.y[w];
-            const double T_sweep = P.T[isw];
-            for (int m0 = 0; m0 < n_omega; m0 += 32) {
-                const int nb = min(32, n_omega - m0);
-                // ---- proposals (row A2): this walker's moves m0 .. m0+nb-1, G per pass ----------------------
-#pragma unroll 1
-                for (int k = sub; k < nb; k += G)
-                    propose_mask(P, (uint32_t)w, (uint32_t)(P.sweep0 + isw), (uint32_t)(m0 + k), y_sweep, T_sweep,
-                                 s_ratio, s_invd, s_wm, rec_gen + k * kRecMaskBytes);
-                __syncwarp();
-
-                int cur = 0;                           // next move of this walker's batch (uniform in the group)
-                while (true) {
-                    // ---- positivity screen (row A3) of the window that holds the cursor ----------------------
-                    int m = 0;
-                    double apn, asn;
-                    bool active;
-                    while (true) {
-                        active = cur < nb;
-                        const int base = active ? (cur & ~(G - 1)) : 0;
-                        const int idx = base + sub;
-                        const uint32_t rq = rbase + (uint32_t)(idx * kRecMaskBytes);
-                        const int4 q0 = lds_s32x4(rq);
-                        const double2 qd = lds_f64x2(rq + 16);
-                        const double a_p = ldg_f64(elem_ptr(a_all, wbase + (uint32_t)q0.x));
-                        const double a_s = ldg_f64(elem_ptr(a_all, wbase + (uint32_t)q0.y));
-                        const double qa = __hiloint2double(q0.w, q0.z);
-                        const double gn = fma(qa, g, g);
-                        apn = fma(gn, a_p, qd.x);
-                        asn = fma(gn, a_s, qd.y);
-                        const bool in_play = active && idx >= cur && idx < nb;
-                        const bool feas = in_play && ((__double2hiint(apn) | __double2hiint(asn)) >= 0);
-                        const uint32_t gb = (__ballot_sync(0xffffffffu, feas) >> gshift) & GM;
-                        const bool exhausted = active && gb == 0u;
-                        const int wend = min(base + G, nb);
-                        if (TRACE) {
-                            // moves of this window that are passed over as infeasible: [cur, m) or [cur, wend)
-                            const int upto = exhausted ? wend : (gb ? base + __ffs((int)gb) - 1 : cur);
-                            if (active && idx >= cur && idx < upto && w < P.W) {
-                                const double2 qt = lds_f64x2(rq + 64);
-                                const size_t mv = ((size_t)(P.call_off + isw)) * n_omega + m0 + idx;
-                                if (P.flags) P.flags[(size_t)w * P.call_sweeps * n_omega + mv] = (uint8_t)0;
-                                if (tracing) {
-                                    sail_trace_rec *tr = P.trace + ((size_t)(w - P.trace_lo) * P.call_sweeps * n_omega + mv);
-                                    tr->p = q0.x; tr->s = q0.y; tr->flags = 0; tr->move = m0 + idx;
-                                    tr->rho = 1.0 + qa; tr->delta_p = qd.x; tr->delta_s = qd.y;
-                                    tr->dchi2 = 0.0; tr->thr = qt.x; tr->ap_new = apn; tr->as_new = asn;
-                                }
-                            }
-                        }
-                        if (exhausted) cur = wend;
-                        else if (gb) m = base + __ffs((int)gb) - 1;
-                        if (!__any_sync(0xffffffffu, exhausted && cur < nb)) { active = cur < nb; break; }
-                    }
-                    if (!__any_sync(0xffffffffu, active)) break;
-
-                    // ---- incremental Delta chi^2 over all tau (row A4) for the move m of every walker ----------
-                    const uint32_t r = rbase + (uint32_t)(m * kRecMaskBytes);
-                    const int4 r0 = lds_s32x4(r);
-                    const double2 dd = lds_f64x2(r + 16);
-                    const double2 dr = lds_f64x2(r + 32);
-                    const double2 sc = lds_f64x2(r + 48);
-                    const double2 th = lds_f64x2(r + 64);
-                    const double alpha = __hiloint2double(r0.w, r0.z);
-                    double e0p, e0s;
-                    if (FACT) {
-                        e0p = lds_f64(e0_lane + (uint32_t)((r0.x >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.x & fmask) * (G * 8)));
-                        e0s = lds_f64(e0_lane + (uint32_t)((r0.y >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.y & fmask) * (G * 8)));
-                    } else {
-                        e0p = lds_f64(e0_lane + (uint32_t)(r0.x * (G * 8)));
-                        e0s = lds_f64(e0_lane + (uint32_t)(r0.y * (G * 8)));
-                    }
-                    double vm = fma(dd.x, e0p, dd.y * e0s);
-                    double vc = fma(dr.x, e0p, dr.y * e0s);
-                    double acc_a = 0.0, acc_b = 0.0;
-#pragma unroll
-                    for (int i = 0; i < C; ++i) {
-                        double vi;
-                        if (i == 0) vi = vm;
-                        else if (i == 1) vi = vc;
-                        else { vi = fma(sc.x, vc, sc.y * vm); vm = vc; vc = vi; }
-                        d[i] = fma(alpha, mt[i], vi);
-                        const double t = fma(Wt[i], d[i], G2[i]);
-                        if (i & 1) acc_b = fma(d[i], t, acc_b);
-                        else       acc_a = fma(d[i], t, acc_a);
-                    }
-                    double dchi2 = (C > 1) ? acc_a + acc_b : acc_a;
-#pragma unroll
-                    for (int off = G / 2; off > 0; off >>= 1) dchi2 += __shfl_xor_sync(0xffffffffu, dchi2, off);
-                    // ---- Metropolis (row A5, Eq. 10), per walker; updates are predicated, not branched --------
-                    const bool acc = active && (dchi2 < th.x);
-                    const int ia = acc ? 1 : 0;
-                    if (__any_sync(0xffffffffu, acc)) {
-#pragma unroll
-                        for (int i = 0; i < C; ++i) {
-                            add_if(mt[i], d[i], ia);
-                            if (W2REG) fma_if(G2[i], W2[i], d[i], ia);
-                            else       fma_if(G2[i], Wt[i], d[i] + d[i], ia);
-                        }
-                        add_if(chi2, dchi2, ia);
-                        fma_if(g, alpha, g, ia);
-                        mul_if(ginv, th.y, ia);
-                        const int mine = (acc && sub == (m & (G - 1))) ? 1 : 0;
-                        stg_f64_if(elem_ptr(a_all, wbase + (uint32_t)r0.x), apn * ginv, mine);
-                        stg_f64_if(elem_ptr(a_all, wbase + (uint32_t)r0.y), asn * ginv, mine);
-                        acc_sweep += ia;
-                    }
-                    eval_sweep += active ? 1 : 0;
-                    if (TRACE) {
-                        if (active && sub == (m & (G - 1)) && w < P.W) {
-                            const int fl = 5 | (ia << 1);
-                            const size_t mv = ((size_t)(P.call_off + isw)) * n_omega + m0 + m;
-                            if (P.flags) P.flags[(size_t)w * P.call_sweeps * n_omega + mv] = (uint8_t)fl;
-                            if (tracing) {
-                                sail_trace_rec *tr = P.trace + ((size_t)(w - P.trace_lo) * P.call_sweeps * n_omega + mv);
-                                tr->p = r0.x; tr->s = r0.y; tr->flags = fl; tr->move = m0 + m;
-                                tr->rho = 1.0 + alpha; tr->delta_p = dd.x; tr->delta_s = dd.y;
-                                tr->dchi2 = dchi2; tr->thr = th.x; tr->ap_new = apn; tr->as_new = asn;
-                            }
-                        }
-                    }
-                    if (active) cur = m + 1;
-                    __syncwarp();
-                }
-                __syncwarp();
-            }
-            // ---- end of sweep: fold the lazy scale (Eq. 19), counters, y (row A6, Eq. 30) ----------------
-            for (int k = sub; k < n_omega; k += G) a_all[(size_t)wbase + k] *= g;
-            g = 1.0;
-            ginv = 1.0;
-            if (sub == 0) {
-                P.n_acc[w] += (unsigned long long)acc_sweep;
-                P.n_eval[w] += (unsigned long long)eval_sweep;
-                P.y[w] = amp_factor(P, acc_sweep, y_sweep);
-            }
-            __syncwarp();
-        }
-#pragma unroll
-        for (int i = 0; i < C; ++i) {
-            const int j = sub + G * i;
-            if (j < P.n_tau) P.mt[(size_t)w * P.n_tau + j] = mt[i];
-        }
-        if (sub == 0) P.chi2[w] = chi2;
-        __syncwarp();
-    }
-}
-
 // ---- sweep tables: ratio[k] = exp(-omega_k G dtau); invd[k] = 1/(k domega); start values E0 ----------
 __global__ void sweep_tables_kernel(int n_omega, int G, double domega, double tau0, double dtau,
                                     const double *omega, int fact, int shift, int n_hi, int n_lo,
@@ -1046,15 +487,14 @@ int ensure_sweep_tables(sail_handle *h, int G)
 }
 
 // ---- dispatch -----------------------------------------------------------------------------------------
-// MODE 0: sub-warp groups / software pipeline (sweep_kernel), 1: lean one walker per warp (sweep_kernel_warp),
-//      2: screened one walker per warp (sweep_kernel_mask), 3: the same with 2 Wj in registers,
-//      4: screened sub-warp groups (sweep_kernel_sub), 5: the same with 2 Wj in registers
-template <int G, int C, int MAXW, bool FACT, bool TRACE, int MODE = 0>
+// MODE 1: lean one walker per warp (sweep_kernel_warp), 2: screened one walker per warp (sweep_kernel_mask),
+//      3: the same with 2 Wj in registers
+template <int C, int MAXW, bool FACT, bool TRACE, int MODE, bool DMMA = false>
 static int launch_variant(sail_handle *h, SweepArgs &args)
 {
-    constexpr int NW = 32 / G;
-    constexpr int rec_bytes = (MODE >= 4) ? NW * kRecMaskBytes : (MODE >= 2) ? kRecMaskBytes : kRecBytes;
-    args.n_groups = (args.W + NW - 1) / NW;
+    constexpr int G = 32;
+    constexpr int rec_bytes = (MODE >= 2) ? kRecMaskBytes : kRecBytes;
+    args.n_groups = args.W;
     int warps = (int)((args.n_groups + h->num_sms - 1) / h->num_sms);
     if (warps > MAXW) warps = MAXW;
     if (warps < 1) warps = 1;
@@ -1066,24 +506,22 @@ static int launch_variant(sail_handle *h, SweepArgs &args)
     if (smem > 227 * 1024)
         return set_err(h, SAIL_ERR_ARG, "sweep tables need %zu bytes of shared memory (> 227 KB)", smem);
     void (*kern)(const SweepArgs);
-    if constexpr (MODE == 5) kern = sweep_kernel_sub<G, C, MAXW, FACT, TRACE, true>;
-    else if constexpr (MODE == 4) kern = sweep_kernel_sub<G, C, MAXW, FACT, TRACE, false>;
-    else if constexpr (MODE == 3) kern = sweep_kernel_mask<C, MAXW, FACT, TRACE, true>;
-    else if constexpr (MODE == 2) kern = sweep_kernel_mask<C, MAXW, FACT, TRACE, false>;
-    else if constexpr (MODE == 1) kern = sweep_kernel_warp<C, MAXW, FACT, TRACE>;
-    else kern = sweep_kernel<G, C, MAXW, FACT, TRACE>;
+    if constexpr (MODE == 3) kern = sweep_kernel_mask<C, MAXW, FACT, TRACE, true, DMMA>;
+    else if constexpr (MODE == 2) kern = sweep_kernel_mask<C, MAXW, FACT, TRACE, false, DMMA>;
+    else kern = sweep_kernel_warp<C, MAXW, FACT, TRACE>;
     SAIL_CUDA_OK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int resident = 0;
     SAIL_CUDA_OK(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, warps * 32, smem));
     if (resident < 1)
-        return set_err(h, SAIL_ERR_CUDA, "sweep kernel (mode %d, G=%d, C=%d, MAXW=%d) does not fit one SM at %d warps per CTA", MODE, G, C, MAXW, warps);
+        return set_err(h, SAIL_ERR_CUDA, "sweep kernel (mode %d, C=%d, MAXW=%d) does not fit one SM at %d warps per CTA", MODE, C, MAXW, warps);
     kern<<<(unsigned)ctas, warps * 32, smem, h->stream>>>(args);
     SAIL_LAUNCH_OK(h, "sweep_kernel");
     return SAIL_OK;
 }
 
 // lanes_per_walker (a tuning knob, see include/sail.h): 0 / 32 = screened one-walker-per-warp kernel (default),
-// 34 = the unscreened lean form, 33 = software-pipelined form, 8 / 16 = sub-warp groups
+// 35 = the same with the other register trade-off, 34 = the unscreened lean form,
+// 8 / 16 = grouped screened kernel (several walkers per warp), 36 = its 32-lane instance
 static int pick_lanes(int requested)
 {
     if (requested == 8 || requested == 16) return requested;
@@ -1094,8 +532,8 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
                   int64_t sweeps_in_call, int64_t call_offset)
 {
     const int req = p->lanes_per_walker;
-    if (!(req == 0 || req == 8 || req == 16 || (req >= 32 && req <= 35)))
-        return set_err(h, SAIL_ERR_ARG, "lanes_per_walker=%d is not one of 0, 8, 16, 32..35", req);
+    if (!(req == 0 || req == 8 || req == 16 || req == 32 || (req >= 34 && req <= 37)))
+        return set_err(h, SAIL_ERR_ARG, "lanes_per_walker=%d is not one of 0, 8, 16, 32, 34..37", req);
     const int G = pick_lanes(req);
     const int C = (h->n_tau + G - 1) / G;
     if (C > 16) return set_err(h, SAIL_ERR_ARG, "n_tau=%d needs more than 16 tau-points per lane at %d lanes", h->n_tau, G);
@@ -1125,45 +563,43 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     a.call_sweeps = sweeps_in_call; a.call_off = call_offset;
     const bool trace = (p->trace != nullptr) || (p->flags != nullptr);
 
-#define SAIL_VARIANT(GG, CC, MW, MODE)                                                                                  \
+    // grouped screened kernel (sweep_grp.cu): 8 / 16 lanes per walker, 36 = its one-walker-per-warp instance
+    if (req == 8 || req == 16 || req == 36) return launch_sweep_grp(h, a, G, C, trace, 0);
+
+#define SAIL_VARIANT(CC, MW, MODE)                                                                                  \
     {                                                                                                                   \
-        if (a.fact) return trace ? launch_variant<GG, CC, MW, true, true, MODE>(h, a) : launch_variant<GG, CC, MW, true, false, MODE>(h, a);   \
-        return trace ? launch_variant<GG, CC, MW, false, true, MODE>(h, a) : launch_variant<GG, CC, MW, false, false, MODE>(h, a);             \
+        if (a.fact) return trace ? launch_variant<CC, MW, true, true, MODE>(h, a) : launch_variant<CC, MW, true, false, MODE>(h, a);   \
+        return trace ? launch_variant<CC, MW, false, true, MODE>(h, a) : launch_variant<CC, MW, false, false, MODE>(h, a);             \
     }
-    if (G == 32 && (req == 0 || req == 32)) {          // screened (default)
-        if (C <= 4) SAIL_VARIANT(32, 4, 28, 2)
-        if (C <= 7) SAIL_VARIANT(32, 7, 16, 3)
-        if (C <= 8) SAIL_VARIANT(32, 8, 16, 3)
-        SAIL_VARIANT(32, 16, 12, 2)
+#define SAIL_VARIANT_D(CC, MW, MODE)                                                                                \
+    {                                                                                                                   \
+        if (a.fact) return trace ? launch_variant<CC, MW, true, true, MODE, true>(h, a) : launch_variant<CC, MW, true, false, MODE, true>(h, a);   \
+        return trace ? launch_variant<CC, MW, false, true, MODE, true>(h, a) : launch_variant<CC, MW, false, false, MODE, true>(h, a);             \
     }
-    if (G == 32 && req == 35) {                        // screened, the other register trade-off
-        if (C <= 4) SAIL_VARIANT(32, 4, 24, 3)
-        if (C <= 7) SAIL_VARIANT(32, 7, 16, 2)
-        if (C <= 8) SAIL_VARIANT(32, 8, 16, 2)
-        SAIL_VARIANT(32, 16, 8, 3)
+    if (req == 37) {                                   // screened, DMMA reduction
+        if (C <= 4) SAIL_VARIANT_D(4, 28, 2)
+        if (C <= 7) SAIL_VARIANT_D(7, 16, 3)
+        if (C <= 8) SAIL_VARIANT_D(8, 16, 3)
+        SAIL_VARIANT_D(16, 12, 2)
     }
-    if (G == 32 && req == 34) {                        // unscreened lean form
-        if (C <= 4) SAIL_VARIANT(32, 4, 28, 1)
-        if (C <= 8) SAIL_VARIANT(32, 8, 16, 1)
-        SAIL_VARIANT(32, 16, 12, 1)
+    if (req == 0 || req == 32) {                       // screened (default)
+        if (C <= 4) SAIL_VARIANT(4, 28, 2)
+        if (C <= 7) SAIL_VARIANT(7, 16, 3)
+        if (C <= 8) SAIL_VARIANT(8, 16, 3)
+        SAIL_VARIANT(16, 12, 2)
     }
-    if (G == 32) {                                     // req == 33: software-pipelined form
-        if (C <= 4) SAIL_VARIANT(32, 4, 16, 0)
-        if (C <= 8) SAIL_VARIANT(32, 8, 12, 0)
-        SAIL_VARIANT(32, 16, 8, 0)
+    if (req == 35) {                                   // screened, the other register trade-off
+        if (C <= 4) SAIL_VARIANT(4, 24, 3)
+        if (C <= 7) SAIL_VARIANT(7, 16, 2)
+        if (C <= 8) SAIL_VARIANT(8, 16, 2)
+        SAIL_VARIANT(16, 8, 3)
     }
-    if (G == 16) {
-        if (C <= 4) SAIL_VARIANT(16, 4, 16, 5)
-        if (C <= 7) SAIL_VARIANT(16, 7, 16, 5)
-        if (C <= 8) SAIL_VARIANT(16, 8, 16, 5)
-        if (C <= 13) SAIL_VARIANT(16, 13, 8, 5)
-        SAIL_VARIANT(16, 16, 8, 5)
-    }
-    if (C <= 4) SAIL_VARIANT(8, 4, 16, 5)
-    if (C <= 8) SAIL_VARIANT(8, 8, 12, 5)
-    if (C <= 13) SAIL_VARIANT(8, 13, 8, 5)
-    SAIL_VARIANT(8, 16, 8, 5)
+    // req == 34: unscreened lean form
+    if (C <= 4) SAIL_VARIANT(4, 28, 1)
+    if (C <= 8) SAIL_VARIANT(8, 16, 1)
+    SAIL_VARIANT(16, 12, 1)
 #undef SAIL_VARIANT
+#undef SAIL_VARIANT_D
 }
 
 } // namespace sail
