@@ -289,6 +289,8 @@ def main_ours(args):
                 "chi2_final_median": float(np.median(chi2_final))}
         if args.extra and world == 1:
             try:
+                from paper_1609_07936_b200.binding import microbench
+                line["microbench"] = microbench(local_rank)
                 line["other_workloads"] = extra_workloads(torch, Sail, local_rank, peaks)
             except Exception as ex:  # supplementary only
                 line["other_workloads"] = {"error": repr(ex)}
@@ -343,6 +345,14 @@ def extra_workloads(torch, Sail, dev_index, peaks):
     hbm = peaks.get("hbm_gbs", 6553.3)
     out["stress_branch_t1"] = {"seconds": t_br, "recipients": int(info2.n_recipients), "algorithmic_GB": algo_bytes / 1e9,
                                "achieved_GBps": algo_bytes / t_br / 1e9, "frac_of_measured_hbm": algo_bytes / t_br / 1e9 / hbm}
+    # the paper's default imprint strength t = 0.1: donor read + recipient read + recipient write
+    info3, _, _ = s.branch(T, 0.1)
+    t_b2 = timed(lambda: s.branch_async(T, 0.1))
+    info4, _, _ = s.branch(T, 0.1)
+    n_rec = 0.5 * (info3.n_recipients + info4.n_recipients)         # the population changes between events
+    algo2 = 16 * w.W + n_rec * state * 3
+    out["stress_branch_t0.1"] = {"seconds": t_b2, "recipients": n_rec, "algorithmic_GB": algo2 / 1e9,
+                                 "achieved_GBps": algo2 / t_b2 / 1e9, "frac_of_measured_hbm": algo2 / t_b2 / 1e9 / hbm}
     s.close()
     return out
 

@@ -187,6 +187,19 @@ SAIL_API int64_t sail_launch_count(const sail_t *h);
  */
 SAIL_API int sail_measure_fp64_peak(int32_t device, void *stream, double *dfma_per_s);
 
+/*
+ * sail_microbench — issue rates and latencies of the units the sweep kernel (rows A2-A6) leans on, measured on
+ * `device` with one CTA per SM (DESIGN.md 6.1 cites them).  `out` is a HOST array of n_out >= SAIL_MICROBENCH_N
+ * doubles, filled as (clk = the device's maximum SM clock):
+ *   [0] DFMA warp-instructions / clk / SM at 8 warps per sub-partition   [1] DMMA m8n8k4 / clk / SM
+ *   [2] clk per SM for (2 DMMA + 8 DFMA) issued together: 2/[1] + 8/[0] means DMMA has no pipe of its own
+ *   [3] SHFL / clk / SM   [4] LDS.128, one address per warp, / clk / SM   [5] LDS.64, lane-contiguous, / clk / SM
+ *   [6] [7] [8] dependent-issue latency of DFMA, SHFL, DMMA in clk       [9] as [0] at ONE warp per sub-partition
+ * Returns SAIL_ERR_ARG for a NULL / short array, SAIL_ERR_CUDA without a device.
+ */
+#define SAIL_MICROBENCH_N 10
+SAIL_API int sail_microbench(int32_t device, void *stream, double *out, int32_t n_out);
+
 #ifdef __cplusplus
 }
 #endif

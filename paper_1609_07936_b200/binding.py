@@ -18,7 +18,7 @@ SAIL_OK, SAIL_ERR_ARG, SAIL_ERR_GRID, SAIL_ERR_ALLOC, SAIL_ERR_CUDA, SAIL_ERR_ST
 
 EXPORTS = ["sail_workspace_bytes", "sail_create", "sail_init_walkers", "sail_anneal", "sail_branch",
            "sail_resync", "sail_get", "sail_get_model", "sail_stats", "sail_set_walkers", "sail_set_sweep",
-           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak"]
+           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak", "sail_microbench"]
 
 
 class SailError(RuntimeError):
@@ -78,6 +78,7 @@ def lib():
         L.sail_launch_count.restype = C.c_int64
         L.sail_launch_count.argtypes = [C.c_void_p]
         L.sail_measure_fp64_peak.argtypes = [C.c_int32, C.c_void_p, C.POINTER(C.c_double)]
+        L.sail_microbench.argtypes = [C.c_int32, C.c_void_p, C.POINTER(C.c_double), C.c_int32]
         _lib = L
     return _lib
 
@@ -98,6 +99,21 @@ def measure_fp64_peak(device=0):
     if rc:
         raise SailError(rc, lib().sail_last_error(None).decode())
     return out.value
+
+
+MICROBENCH_KEYS = ("dfma_per_clk_sm", "dmma_m8n8k4_per_clk_sm", "clk_per_sm_2dmma_8dfma", "shfl_per_clk_sm",
+                   "lds128_uniform_per_clk_sm", "lds64_lane_per_clk_sm", "dfma_latency_clk", "shfl_latency_clk",
+                   "dmma_latency_clk", "dfma_per_clk_sm_1warp_per_subpartition")
+
+
+def microbench(device=0):
+    """Issue rates / latencies behind the sweep-kernel design (include/sail.h: sail_microbench)."""
+    import torch
+    out = (C.c_double * len(MICROBENCH_KEYS))()
+    rc = lib().sail_microbench(device, C.c_void_p(torch.cuda.current_stream(device).cuda_stream), out, len(MICROBENCH_KEYS))
+    if rc:
+        raise SailError(rc, lib().sail_last_error(None).decode())
+    return {k: float(v) for k, v in zip(MICROBENCH_KEYS, out)}
 
 
 class Sail:

@@ -158,6 +158,11 @@ __global__ void donor_map_kernel(long long W, const int32_t *__restrict__ mult, 
 
 // Eq. 26: a(l1) <- t a(l2) + (1-t) a(l1) for spectrum and model (linearity); chi^2 of the
 // recipient from its new model.  One CTA per recipient, 128-bit accesses when rows are 16-byte aligned.
+// One CTA per recipient: a and mt of the recipient become t * donor + (1 - t) * self (two roundings per product
+// and one per sum, exactly the definition), chi^2 is recomputed from the new model.  COPY (t == 1): t * z + 0 * x
+// is z bit for bit, so the recipient is not read at all (two streams instead of three).  All loads of a CTA's
+// pass are issued before its first store (8 x 16 B per thread in flight).
+template <bool COPY>
 __global__ void __launch_bounds__(256) imprint_kernel(int n_omega, int n_tau, double t, const int64_t *__restrict__ rec_list,
                                                       const int64_t *__restrict__ donor_of, const unsigned long long *scalars,
                                                       double *a, double *mt, double *chi2,
@@ -166,27 +171,37 @@ __global__ void __launch_bounds__(256) imprint_kernel(int n_omega, int n_tau, do
     __shared__ double red[8];
     const long long n_rec = (long long)scalars[2];
     const double omt = 1.0 - t;
+    auto mix = [&](double z, double x) { return COPY ? z : __dadd_rn(__dmul_rn(t, z), __dmul_rn(omt, x)); };
     for (long long r = blockIdx.x; r < n_rec; r += gridDim.x) {
         const long long i = rec_list[r], dn = donor_of[i];
         double *ai = a + (size_t)i * n_omega;
         const double *ad = a + (size_t)dn * n_omega;
+        double *mi = mt + (size_t)i * n_tau;
+        const double *md = mt + (size_t)dn * n_tau;
         if ((n_omega & 1) == 0) {
             double2 *ai2 = reinterpret_cast<double2 *>(ai);
             const double2 *ad2 = reinterpret_cast<const double2 *>(ad);
-            for (int k = threadIdx.x; k < n_omega / 2; k += blockDim.x) {
-                const double2 x = ai2[k], z = ad2[k];
-                ai2[k] = make_double2(__dadd_rn(__dmul_rn(t, z.x), __dmul_rn(omt, x.x)),
-                                      __dadd_rn(__dmul_rn(t, z.y), __dmul_rn(omt, x.y)));
+            const int n2 = n_omega / 2;
+            constexpr int U = COPY ? 8 : 4;          // 8 x 16 B per thread in flight either way
+            for (int k0 = threadIdx.x; k0 < n2; k0 += U * 256) {
+                double2 x[U], z[U];
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const int k = k0 + u * 256;
+                    if (k < n2) { z[u] = ad2[k]; if (!COPY) x[u] = ai2[k]; }
+                }
+#pragma unroll
+                for (int u = 0; u < U; ++u) {
+                    const int k = k0 + u * 256;
+                    if (k < n2) ai2[k] = make_double2(mix(z[u].x, COPY ? 0.0 : x[u].x), mix(z[u].y, COPY ? 0.0 : x[u].y));
+                }
             }
         } else {
-            for (int k = threadIdx.x; k < n_omega; k += blockDim.x)
-                ai[k] = __dadd_rn(__dmul_rn(t, ad[k]), __dmul_rn(omt, ai[k]));
+            for (int k = threadIdx.x; k < n_omega; k += blockDim.x) ai[k] = mix(ad[k], COPY ? 0.0 : ai[k]);
         }
-        double *mi = mt + (size_t)i * n_tau;
-        const double *md = mt + (size_t)dn * n_tau;
         double s = 0.0;
         for (int j = threadIdx.x; j < n_tau; j += blockDim.x) {
-            const double v = __dadd_rn(__dmul_rn(t, md[j]), __dmul_rn(omt, mi[j]));
+            const double v = mix(md[j], COPY ? 0.0 : mi[j]);
             mi[j] = v;
             const double D = v - fj[j];
             s = fma(Wj[j] * D, D, s);
@@ -225,8 +240,12 @@ int launch_branch(sail_handle *h, double T, double t_imprint)
     donor_map_kernel<<<blocks, 256, 0, h->stream>>>(W, b.mult, b.scanA, b.scanB, b.donor_of, b.rec_list, b.scalars);
     SAIL_LAUNCH_OK(h, "donor_map_kernel");
     const int iblocks = (int)(W < (long long)h->num_sms * 8 ? W : (long long)h->num_sms * 8);
-    imprint_kernel<<<iblocks, 256, 0, h->stream>>>(h->n_omega, h->n_tau, t_imprint, b.rec_list, b.donor_of, b.scalars,
-                                                   h->st.a, h->st.mt, h->st.chi2, h->tab.Wj, h->tab.fj);
+    if (t_imprint == 1.0)
+        imprint_kernel<true><<<iblocks, 256, 0, h->stream>>>(h->n_omega, h->n_tau, t_imprint, b.rec_list, b.donor_of, b.scalars,
+                                                             h->st.a, h->st.mt, h->st.chi2, h->tab.Wj, h->tab.fj);
+    else
+        imprint_kernel<false><<<iblocks, 256, 0, h->stream>>>(h->n_omega, h->n_tau, t_imprint, b.rec_list, b.donor_of, b.scalars,
+                                                              h->st.a, h->st.mt, h->st.chi2, h->tab.Wj, h->tab.fj);
     SAIL_LAUNCH_OK(h, "imprint_kernel");
     return SAIL_OK;
 }

@@ -519,8 +519,9 @@ static int launch_variant(sail_handle *h, SweepArgs &args)
     return SAIL_OK;
 }
 
-// lanes_per_walker (a tuning knob, see include/sail.h): 0 / 32 = screened one-walker-per-warp kernel (default),
-// 35 = the same with the other register trade-off, 34 = the unscreened lean form,
+// lanes_per_walker (a tuning knob, see include/sail.h): 0 / 32 = screened one-walker-per-warp kernel with the DMMA
+// warp sum (default), 35 = the same with the other register trade-off, 37 = the same with the shuffle butterfly,
+// 34 = the unscreened lean form,
 // 8 / 16 = grouped screened kernel (several walkers per warp), 36 = its 32-lane instance
 static int pick_lanes(int requested)
 {
@@ -576,23 +577,23 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
         if (a.fact) return trace ? launch_variant<CC, MW, true, true, MODE, true>(h, a) : launch_variant<CC, MW, true, false, MODE, true>(h, a);   \
         return trace ? launch_variant<CC, MW, false, true, MODE, true>(h, a) : launch_variant<CC, MW, false, false, MODE, true>(h, a);             \
     }
-    if (req == 37) {                                   // screened, DMMA reduction
+    if (req == 0 || req == 32) {                       // screened, DMMA warp sum (default)
         if (C <= 4) SAIL_VARIANT_D(4, 28, 2)
         if (C <= 7) SAIL_VARIANT_D(7, 16, 3)
         if (C <= 8) SAIL_VARIANT_D(8, 16, 3)
         SAIL_VARIANT_D(16, 12, 2)
     }
-    if (req == 0 || req == 32) {                       // screened (default)
+    if (req == 35) {                                   // the same, the other register trade-off
+        if (C <= 4) SAIL_VARIANT_D(4, 24, 3)
+        if (C <= 7) SAIL_VARIANT_D(7, 16, 2)
+        if (C <= 8) SAIL_VARIANT_D(8, 16, 2)
+        SAIL_VARIANT_D(16, 8, 3)
+    }
+    if (req == 37) {                                   // screened, shuffle-butterfly warp sum
         if (C <= 4) SAIL_VARIANT(4, 28, 2)
         if (C <= 7) SAIL_VARIANT(7, 16, 3)
         if (C <= 8) SAIL_VARIANT(8, 16, 3)
         SAIL_VARIANT(16, 12, 2)
-    }
-    if (req == 35) {                                   // screened, the other register trade-off
-        if (C <= 4) SAIL_VARIANT(4, 24, 3)
-        if (C <= 7) SAIL_VARIANT(7, 16, 2)
-        if (C <= 8) SAIL_VARIANT(8, 16, 2)
-        SAIL_VARIANT(16, 8, 3)
     }
     // req == 34: unscreened lean form
     if (C <= 4) SAIL_VARIANT(4, 28, 1)

@@ -382,3 +382,13 @@ def test_single_tau_and_single_walker_degenerate_cases():
     a, _ = s.get()
     np.testing.assert_allclose(a, o.a, rtol=0, atol=1e-12)
     s.close()
+
+
+def test_microbench_reports_the_unit_rates_the_design_cites():
+    """sail_microbench (include/sail.h): sanity of the measured issue rates."""
+    from paper_1609_07936_b200.binding import microbench
+    m = microbench(0)
+    assert 1.5 < m["dfma_per_clk_sm"] < 2.2             # 64 FP64 lanes per SM = 2 warp-instructions per clock
+    assert 0.15 < m["dmma_m8n8k4_per_clk_sm"] < 0.6
+    assert 0.5 < m["shfl_per_clk_sm"] < 1.3
+    assert all(v > 0 for v in m.values())
