@@ -95,8 +95,8 @@ def measured_peaks():
 
 
 # dram__bytes_read.sum + dram__bytes_write.sum of one sweep-kernel launch, from the committed ncu --set full capture
-# (profiles/r01_sweep_small_full_metrics.txt): 12.09 MB + 2.35 MB for the whole 5000-sweep Small anneal
-SWEEP_DRAM_BYTES_PER_LAUNCH = {("small", 5000): 14.44e6}
+# (profiles/r01_sweep_small_full_metrics.txt): 12.06 MB + 3.07 MB for the whole 5000-sweep Small anneal
+SWEEP_DRAM_BYTES_PER_LAUNCH = {("small", 5000): 15.13e6}
 
 LANES = 0   # --lanes: lanes of a warp per walker (0 = library default)
 
