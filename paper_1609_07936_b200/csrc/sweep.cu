@@ -533,13 +533,15 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
                   int64_t sweeps_in_call, int64_t call_offset)
 {
     const int req = p->lanes_per_walker;
-    if (!(req == 0 || req == 8 || req == 16 || req == 32 || (req >= 34 && req <= 37)))
-        return set_err(h, SAIL_ERR_ARG, "lanes_per_walker=%d is not one of 0, 8, 16, 32, 34..37", req);
+    if (!(req == 0 || req == 1 || req == 8 || req == 16 || req == 32 || (req >= 34 && req <= 37)))
+        return set_err(h, SAIL_ERR_ARG, "lanes_per_walker=%d is not one of 0, 1, 8, 16, 32, 34..37", req);
     const int G = pick_lanes(req);
     const int C = (h->n_tau + G - 1) / G;
-    if (C > 16) return set_err(h, SAIL_ERR_ARG, "n_tau=%d needs more than 16 tau-points per lane at %d lanes", h->n_tau, G);
-    int rc = ensure_sweep_tables(h, G);
-    if (rc) return rc;
+    if (req != 1) {
+        if (C > 16) return set_err(h, SAIL_ERR_ARG, "n_tau=%d needs more than 16 tau-points per lane at %d lanes", h->n_tau, G);
+        int rc = ensure_sweep_tables(h, G);
+        if (rc) return rc;
+    }
     const long long W_pad = (h->W + 3) & ~3LL;
     if ((unsigned long long)W_pad * (unsigned long long)h->n_omega >= (1ull << 32))
         return set_err(h, SAIL_ERR_ARG, "W * n_omega must be < 2^32 spectral coefficients");
@@ -564,6 +566,7 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     a.call_sweeps = sweeps_in_call; a.call_off = call_offset;
     const bool trace = (p->trace != nullptr) || (p->flags != nullptr);
 
+    if (req == 1) return launch_sweep_lw(h, a, trace, h->h_Wj.data(), h->h_fj.data());   // lane per walker (sweep_lw.cu)
     // grouped screened kernel (sweep_grp.cu): 8 / 16 lanes per walker, 36 = its one-walker-per-warp instance
     if (req == 8 || req == 16 || req == 36) return launch_sweep_grp(h, a, G, C, trace, 0);
 
