@@ -210,10 +210,6 @@ int sail_create(sail_t **out, const double *omega, int32_t n_omega, const double
     rc = launch_problem_tables(h, D(L.off_F), sigma ? D(L.off_sigma) : nullptr, D(L.off_c), D(L.off_Wj), D(L.off_fj), D(L.off_E));
     if (rc) return fail(rc);
     if (cudaStreamSynchronize(h->stream) != cudaSuccess) return fail(set_err(h, SAIL_ERR_CUDA, "table build failed: %s", cudaGetErrorString(cudaGetLastError())));
-    h->h_Wj.resize(n_tau); h->h_fj.resize(n_tau);
-    if (cudaMemcpy(h->h_Wj.data(), h->tab.Wj, n_tau * sizeof(double), cudaMemcpyDeviceToHost) != cudaSuccess ||
-        cudaMemcpy(h->h_fj.data(), h->tab.fj, n_tau * sizeof(double), cudaMemcpyDeviceToHost) != cudaSuccess)
-        return fail(set_err(h, SAIL_ERR_CUDA, "table read-back failed: %s", cudaGetErrorString(cudaGetLastError())));
     *out = h;
     return SAIL_OK;
 }

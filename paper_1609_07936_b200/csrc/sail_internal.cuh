@@ -5,7 +5,6 @@
 #include <stdint.h>
 #include <stdio.h>
 #include <string>
-#include <vector>
 
 #include "../../include/sail.h"
 
@@ -82,8 +81,6 @@ struct sail_handle {
     size_t d_T_cap = 0;
     double *h_pinned = nullptr;  // small pinned staging buffer
     size_t h_pinned_cap = 0;
-
-    std::vector<double> h_Wj, h_fj;   // host copies of the per-tau weights (kernel parameters of the lane-per-walker sweep kernel)
 
     int64_t launches = 0;
     std::string err;

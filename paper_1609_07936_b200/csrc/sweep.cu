@@ -234,7 +234,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
 //    and propagate through the bounded Green's function (r_p^{n+1} - r_s^{n+1})/(r_p - r_s) <= n + 1.
 //  * with W2REG the constants 2 Wj live in registers as well: the accepted update is 2 instructions per
 //    tau-point instead of 3.
-template <int C, int MAXW, bool FACT, bool TRACE, bool W2REG, bool DMMA>
+template <int C, int MAXW, bool FACT, bool TRACE, bool W2REG, int DMMA>
 __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kernel_mask(const SweepArgs P)
 {
     constexpr int G = 32;
@@ -357,7 +357,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                         else       acc_a = fma(d[i], t, acc_a);
                     }
                     double dchi2 = (C > 1) ? acc_a + acc_b : acc_a;
-                    if (DMMA) {
+                    if (DMMA == 1) {
                         dchi2 = warp_sum_dmma(dchi2);
                     } else {
 #pragma unroll
@@ -489,7 +489,7 @@ int ensure_sweep_tables(sail_handle *h, int G)
 // ---- dispatch -----------------------------------------------------------------------------------------
 // MODE 1: lean one walker per warp (sweep_kernel_warp), 2: screened one walker per warp (sweep_kernel_mask),
 //      3: the same with 2 Wj in registers
-template <int C, int MAXW, bool FACT, bool TRACE, int MODE, bool DMMA = false>
+template <int C, int MAXW, bool FACT, bool TRACE, int MODE, int DMMA = 0>
 static int launch_variant(sail_handle *h, SweepArgs &args)
 {
     constexpr int G = 32;
@@ -533,15 +533,13 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
                   int64_t sweeps_in_call, int64_t call_offset)
 {
     const int req = p->lanes_per_walker;
-    if (!(req == 0 || req == 1 || req == 8 || req == 16 || req == 32 || (req >= 34 && req <= 37)))
-        return set_err(h, SAIL_ERR_ARG, "lanes_per_walker=%d is not one of 0, 1, 8, 16, 32, 34..37", req);
+    if (!(req == 0 || req == 8 || req == 16 || req == 32 || (req >= 34 && req <= 37)))
+        return set_err(h, SAIL_ERR_ARG, "lanes_per_walker=%d is not one of 0, 8, 16, 32, 34..37", req);
     const int G = pick_lanes(req);
     const int C = (h->n_tau + G - 1) / G;
-    if (req != 1) {
-        if (C > 16) return set_err(h, SAIL_ERR_ARG, "n_tau=%d needs more than 16 tau-points per lane at %d lanes", h->n_tau, G);
-        int rc = ensure_sweep_tables(h, G);
-        if (rc) return rc;
-    }
+    if (C > 16) return set_err(h, SAIL_ERR_ARG, "n_tau=%d needs more than 16 tau-points per lane at %d lanes", h->n_tau, G);
+    int rc = ensure_sweep_tables(h, G);
+    if (rc) return rc;
     const long long W_pad = (h->W + 3) & ~3LL;
     if ((unsigned long long)W_pad * (unsigned long long)h->n_omega >= (1ull << 32))
         return set_err(h, SAIL_ERR_ARG, "W * n_omega must be < 2^32 spectral coefficients");
@@ -566,7 +564,6 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     a.call_sweeps = sweeps_in_call; a.call_off = call_offset;
     const bool trace = (p->trace != nullptr) || (p->flags != nullptr);
 
-    if (req == 1) return launch_sweep_lw(h, a, trace, h->h_Wj.data(), h->h_fj.data());   // lane per walker (sweep_lw.cu)
     // grouped screened kernel (sweep_grp.cu): 8 / 16 lanes per walker, 36 = its one-walker-per-warp instance
     if (req == 8 || req == 16 || req == 36) return launch_sweep_grp(h, a, G, C, trace, 0);
 
@@ -577,8 +574,8 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     }
 #define SAIL_VARIANT_D(CC, MW, MODE)                                                                                \
     {                                                                                                                   \
-        if (a.fact) return trace ? launch_variant<CC, MW, true, true, MODE, true>(h, a) : launch_variant<CC, MW, true, false, MODE, true>(h, a);   \
-        return trace ? launch_variant<CC, MW, false, true, MODE, true>(h, a) : launch_variant<CC, MW, false, false, MODE, true>(h, a);             \
+        if (a.fact) return trace ? launch_variant<CC, MW, true, true, MODE, 1>(h, a) : launch_variant<CC, MW, true, false, MODE, 1>(h, a);   \
+        return trace ? launch_variant<CC, MW, false, true, MODE, 1>(h, a) : launch_variant<CC, MW, false, false, MODE, 1>(h, a);             \
     }
     if (req == 0 || req == 32) {                       // screened, DMMA warp sum (default)
         if (C <= 4) SAIL_VARIANT_D(4, 28, 2)

@@ -151,7 +151,5 @@ __device__ __forceinline__ MoveRegs propose_mask(const SweepArgs &P, uint32_t wa
 
 // implemented in sweep_grp.cu: the grouped screened kernel (G = 8, 16 or 32 lanes per walker)
 int launch_sweep_grp(sail_handle *h, SweepArgs &args, int G, int C, bool trace, int flavour);
-// implemented in sweep_lw.cu: the lane-per-walker kernel (a CTA owns 32 walkers, a warp owns a tau-slice of all of them)
-int launch_sweep_lw(sail_handle *h, SweepArgs &args, bool trace, const double *h_Wj, const double *h_fj);
 
 } // namespace sail

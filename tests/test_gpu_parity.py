@@ -86,7 +86,7 @@ def test_init_forward_and_residue_match_oracle():
     s.close()
 
 
-@pytest.mark.parametrize("lanes", [0, 1, 37, 35, 34, 36, 16, 8])
+@pytest.mark.parametrize("lanes", [0, 37, 35, 34, 36, 16, 8])
 def test_tiny_full_anneal_trace_and_sequence_parity(lanes):
     """configs[0] in full: 64 walkers x 2000 sweeps x 64 moves, every move traced (L1, L2, L3)."""
     w = wl.make("tiny", simpson_intervals=100_000)
@@ -127,7 +127,7 @@ def test_tiny_full_anneal_trace_and_sequence_parity(lanes):
 @pytest.mark.parametrize("name,W,lanes,n_sw", [("small", 97, 32, 12), ("small", 97, 35, 12), ("small", 97, 34, 12), ("small", 97, 16, 12), ("small", 97, 36, 12), ("small", 50, 8, 8),
                                                ("branching", 70, 16, 4), ("branching", 33, 32, 4), ("branching", 33, 35, 4),
                                                ("noise", 40, 32, 3), ("noise", 40, 35, 3), ("noise", 40, 16, 3), ("stress", 35, 32, 2), ("stress", 35, 35, 2),
-                                               ("stress", 35, 34, 2), ("stress", 35, 36, 2), ("noise", 40, 36, 3), ("small", 97, 1, 12), ("branching", 33, 1, 4), ("noise", 40, 1, 3), ("small", 97, 37, 12), ("branching", 33, 37, 4), ("noise", 40, 37, 3), ("stress", 35, 37, 2)])
+                                               ("stress", 35, 34, 2), ("stress", 35, 36, 2), ("noise", 40, 36, 3), ("small", 97, 37, 12), ("branching", 33, 37, 4), ("noise", 40, 37, 3), ("stress", 35, 37, 2)])
 def test_ragged_sizes_trace_parity(name, W, lanes, n_sw):
     """Other configs' grids (N_tau = 100, 200, 256, 512: several tau-points per lane with a ragged tail,
     factored start tables for the large N_omega) at walker counts that do not fill the last warp."""
