@@ -7,6 +7,7 @@
 
 #include <vector>
 
+#include <stdlib.h>
 #include "sail_internal.cuh"
 
 namespace sail {
@@ -210,6 +211,7 @@ int sail_create(sail_t **out, const double *omega, int32_t n_omega, const double
     rc = launch_problem_tables(h, D(L.off_F), sigma ? D(L.off_sigma) : nullptr, D(L.off_c), D(L.off_Wj), D(L.off_fj), D(L.off_E));
     if (rc) return fail(rc);
     if (cudaStreamSynchronize(h->stream) != cudaSuccess) return fail(set_err(h, SAIL_ERR_CUDA, "table build failed: %s", cudaGetErrorString(cudaGetLastError())));
+    h->no_tma_imprint = getenv("SAIL_NO_TMA_IMPRINT") != nullptr;
     *out = h;
     return SAIL_OK;
 }

@@ -82,6 +82,8 @@ struct sail_handle {
     double *h_pinned = nullptr;  // small pinned staging buffer
     size_t h_pinned_cap = 0;
 
+    bool no_tma_imprint = false;   // SAIL_NO_TMA_IMPRINT=1 in the environment at sail_create: plain-load imprint kernel (A/B measurements)
+
     int64_t launches = 0;
     std::string err;
 };
