@@ -27,7 +27,7 @@ int set_err(sail_handle *h, int code, const char *fmt, ...)
 
 // ---- workspace layout ------------------------------------------------------------------------------
 struct Layout {
-    size_t off_omega, off_tau, off_c, off_Wj, off_fj, off_F, off_sigma, off_E, off_ratio, off_invd, off_E0;
+    size_t off_omega, off_tau, off_c, off_Wj, off_fj, off_F, off_sigma, off_E, off_ET, off_ratio, off_invd, off_E0;
     size_t off_a, off_mt, off_chi2, off_y, off_nacc, off_neval;
     size_t off_ehat, off_scanA, off_scanB, off_bsums, off_mult, off_donor, off_reclist, off_scalars;
     size_t total;
@@ -44,6 +44,7 @@ static Layout make_layout(int n_omega, int n_tau, int64_t Wmax)
     L.off_omega = take(n_omega * d);  L.off_tau = take(n_tau * d);   L.off_c = take(n_tau * d);
     L.off_Wj = take(n_tau * d);       L.off_fj = take(n_tau * d);    L.off_F = take(n_tau * d);
     L.off_sigma = take(n_tau * d);    L.off_E = take((size_t)n_omega * n_tau * d);
+    L.off_ET = take((size_t)n_omega * n_tau * d);
     L.off_ratio = take(n_omega * d);  L.off_invd = take(n_omega * d);  L.off_E0 = take(kE0Doubles * d);
     L.off_a = take(W * n_omega * d);  L.off_mt = take(W * n_tau * d);
     L.off_chi2 = take(W * d);         L.off_y = take(W * d);
@@ -194,7 +195,7 @@ int sail_create(sail_t **out, const double *omega, int32_t n_omega, const double
     auto D = [&](size_t off) { return (double *)(base + off); };
     auto U = [&](size_t off) { return (unsigned long long *)(base + off); };
     h->tab.omega = D(L.off_omega); h->tab.tau = D(L.off_tau); h->tab.c = D(L.off_c); h->tab.Wj = D(L.off_Wj);
-    h->tab.fj = D(L.off_fj); h->tab.E = D(L.off_E);
+    h->tab.fj = D(L.off_fj); h->tab.E = D(L.off_E); h->tab.ET = D(L.off_ET);
     h->sw_ratio = D(L.off_ratio); h->sw_invd = D(L.off_invd); h->sw_E0 = D(L.off_E0);
     h->st.a = D(L.off_a); h->st.mt = D(L.off_mt); h->st.chi2 = D(L.off_chi2); h->st.y = D(L.off_y);
     h->st.n_acc = U(L.off_nacc); h->st.n_eval = U(L.off_neval);

@@ -27,6 +27,7 @@ struct DevTables {
     const double *Wj;      // [n_tau]
     const double *fj;      // [n_tau]
     const double *E;       // [n_omega][n_tau] exp(-omega_k tau_j), for the dense forward transform
+    double *ET;            // [n_tau][n_omega] the same, transposed (k contiguous: the B operand of the DMMA forward kernel)
 };
 
 struct DevState {
