@@ -392,3 +392,37 @@ def test_microbench_reports_the_unit_rates_the_design_cites():
     assert 0.15 < m["dmma_m8n8k4_per_clk_sm"] < 0.6
     assert 0.5 < m["shfl_per_clk_sm"] < 1.3
     assert all(v > 0 for v in m.values())
+
+
+@pytest.mark.parametrize("n_omega,n_tau,W", [(37, 11, 45), (50, 33, 70), (130, 257, 33)])
+def test_odd_grid_sizes_take_the_fallback_kernels(n_omega, n_tau, W):
+    """Grids that are not multiples of 2 / 4 (N_omega = 37, 50, 130; N_tau = 11, 33, 257): the forward transform runs on
+    the register-tiled DFMA kernel instead of the DMMA one, the t = 1 imprint on plain loads instead of the bulk-copy
+    engine, the sweep kernel has a ragged last batch and ragged tau tail.  Same parity bars as everywhere else."""
+    w = wl.random_problem(11, n_omega, n_tau)
+    o = _oracle(w, W)
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED)
+    np.testing.assert_allclose(s.get()[0], o.a, rtol=1e-12)
+    s.set_walkers(0, o.a)
+    np.testing.assert_allclose(s.get_model(), o.M, rtol=1e-12)
+    T = wl.geometric_schedule(1.0, 0.5, 4)
+    tg, fg = s.anneal(T, w.eta, trace_walkers=(0, W), want_flags=True)
+    to, fo = o.anneal(T, trace_walkers=(0, W), want_flags=True)
+    assert compare_traces(tg, to, T, w.A / w.n_omega) == 0
+    assert ((fg & 3) == fo).all()
+    a, c2 = s.get()
+    np.testing.assert_allclose(a, o.a, rtol=0, atol=1e-10 * o.a.max())
+    o.a[:] = a; o.chi2[:] = c2
+    for t in (1.0, 0.3):
+        Tb = float(np.std(o.chi2))
+        info, mult, donor = s.branch(Tb, t, want_maps=True)
+        n_rec, mo, do = o.branch(Tb, t)
+        assert (mult == mo).all() and (donor == do).all() and info.n_recipients == n_rec
+        a1, c1 = s.get()
+        np.testing.assert_array_equal(a1, o.a)
+        np.testing.assert_allclose(c1, o.chi2, rtol=1e-8)
+        o.chi2[:] = c1
+    s.resync(); o.resync()
+    np.testing.assert_allclose(s.get(spectra=False)[1], o.chi2, rtol=1e-9)
+    s.close()
