@@ -110,7 +110,11 @@ typedef struct {
 typedef struct {
     double  eta;             /* base amplitude: rho = 1 - y eta (2u - 1), requires 0 < eta < 1 (reading G6) */
     int32_t amp_mode;        /* 0: y = 1;  1: Eq. 30 from the previous sweep's acceptance  */
-    int32_t lanes_per_walker;/* 0 = auto; else 8, 16 or 32 lanes of a warp cooperate on one walker  */
+    int32_t lanes_per_walker;/* sweep-kernel form, a tuning knob (all forms make the same moves and decisions):
+                              * 0 / 32 screened one-walker-per-warp kernel, DMMA warp sum (default);
+                              * 37 the same with the shuffle butterfly; 35 the same, other register budget;
+                              * 34 unscreened form; 8 / 16 lanes per walker: several walkers per warp in
+                              * lockstep; 36 the 32-lane instance of that kernel          */
     double  amp_p, amp_m;    /* Eq. 30 parameters (paper: p = 1, m = 2, :222)                      */
     double  y_min;           /* floor of y (reading G7), e.g. 1e-6                                  */
     int64_t resync_every;    /* full-residual resync after every such absolute sweep; 0 = never    */

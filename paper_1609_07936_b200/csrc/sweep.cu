@@ -1,23 +1,25 @@
-// sweep.cu — the persistent Monte Carlo sweep kernel.
+// sweep.cu — the persistent Monte Carlo sweep kernels with one walker per warp (
+// PAPER.md:127-148, :205) and the dispatch of all sweep-kernel forms.
 //
-// Mapping: G lanes of a warp cooperate on one walker (32/G walkers per warp); lane l
-// owns tau-points j = l + G*i, i < C, whose residual state lives in REGISTERS for the whole launch:
+// Mapping: one walker per warp; lane l owns tau-points j = l + 32 i, i < C, whose residual state
+// lives in REGISTERS for the whole launch:
 //     mt_j  = sum_k a_k exp(-omega_k tau_j)      (model in the pure-exponential basis, M_j = c_j mt_j)
 //     G2_j  = 2 Wj (mt_j - fj)                   (Wj = (c_j/sigma_j)^2, fj = F_j/c_j)
 // so that for a move (p, s, rho, delta_p, delta_s) (Eq. 17-22):
 //     dt_j   = (rho-1) mt_j + delta_p E_pj + delta_s E_sj          E_kj = exp(-omega_k tau_j)
 //     dchi2  = sum_j dt_j (Wj dt_j + G2_j)     [= sum_j d_j (d_j + 2 D_j) of SURVEY §8a row A4]
-// The kernel rows are never read from a table in the inner loop: both grids are uniform (Eq. 2-3, 7),
-// so E_{k,j+G} = E_kj * exp(-omega_k G dtau); each lane starts from E0[k][l] (shared memory) and
-// advances by one DMUL per row per tau-point, with delta folded into the start value:
-//     6 FP64-pipe instructions per tau-point (2 DMUL, 1 DADD, 3 DFMA), no memory traffic.
-// Proposals (Philox4x32-10 keyed by (seed; walker, sweep, move, 0), index draw, rho, Eq. 20-21,
-// -T ln u) do not depend on the chain state within a sweep, so they are computed G moves at a time,
-// one move per lane, and staged as 64-byte records in shared memory.
-// Eq. 19 (scale ALL coefficients by rho) is applied lazily: a = g * a~, g <- g rho on accept, folded
-// into a~ at the end of every sweep.
-// Walker slots W .. W_pad-1 (W_pad = W rounded up to 4) are scratch copies of the last walker so that a
-// warp never has an inactive group: no activity predicate in the hot loop; they are never reported.
+// The kernel rows are never read from a table in the inner loop: both grids are uniform (Eq. 2-3, 7), so
+// E_{k,j+32} = E_kj exp(-omega_k 32 dtau); each lane starts from E0[k][l] (shared memory) and advances by a
+// recurrence along its tau-points.
+//   sweep_kernel_mask (default): positivity screened for a 32-move batch at once (ballot), two-term recurrence for
+//       delta_p E_p + delta_s E_s (5 FP64 per tau-point), warp sum on the DMMA path; see its own comment below;
+//   sweep_kernel_warp: the plain form — every move visited in turn, one geometric recurrence per row (6 FP64 per
+//       tau-point), shuffle butterfly; kept as the simple reference form of the same arithmetic.
+// Proposals (Philox4x32-10 keyed by (seed; walker, sweep, move, 0), index draw, rho, Eq. 20-21, -T ln u) do not
+// depend on the chain state within a sweep, so they are computed 32 moves at a time, one move per lane, and staged
+// as records in shared memory.  Eq. 19 (scale ALL coefficients by rho) is applied lazily: a = g * a~, g <- g rho on
+// accept, folded into a~ at the end of every sweep.  Walker slots W .. W_pad-1 (W_pad = W rounded up to 4) are
+// scratch copies of the last walker (used by the grouped kernel of sweep_grp.cu); they are never reported.
 #include "sweep_common.cuh"
 
 namespace sail {
@@ -53,7 +55,7 @@ __device__ __forceinline__ void propose(const SweepArgs &P, uint32_t walker, uin
 }
 
 // ---- one walker per WARP, register-lean (<= 72 registers: 28 resident warps per SM = 7 per sub-partition) ------
-// Same arithmetic as sweep_kernel<32, C, ...>; no software pipeline (the other six warps of the sub-partition hide
+// No software pipeline (the other six warps of the sub-partition hide
 // the latencies), every decision is warp-uniform, so infeasible and rejected moves branch around the work.
 template <int C, int MAXW, bool FACT, bool TRACE>
 __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kernel_warp(const SweepArgs P)
