@@ -426,3 +426,51 @@ def test_odd_grid_sizes_take_the_fallback_kernels(n_omega, n_tau, W):
     s.resync(); o.resync()
     np.testing.assert_allclose(s.get(spectra=False)[1], o.chi2, rtol=1e-9)
     s.close()
+
+
+@pytest.mark.parametrize("name", ["branching", "noise"])
+def test_branching_and_noise_configurations_sampled_parity(name):
+    """configs[2] (Branching: W = 65536, N_omega = 512, N_tau = 200) and configs[3] (Noise sweep, one anneal:
+    W = 16384, N_omega = 1024, N_tau = 256) at FULL size: one block of the protocol on the GPU (branch_every sweeps,
+    then one imprinted-branching event at t = 0.1), the event checked for what is unique (sum m = W, donors have
+    m >= 2, recipients are exactly t donor + (1 - t) self), then 16 walkers — half of them fresh recipients — traced
+    for one sweep and replayed by the oracle from the injected GPU state."""
+    w = wl.make(name, simpson_intervals=100_000)
+    s = _sail(w, w.W)
+    s.init_walkers(w.W, w.A, w.B, SEED)
+    nb = w.branch_every
+    assert nb > 0
+    s.anneal(w.schedule[:nb], w.eta)
+    a0, c0 = s.get()
+    t = w.t_imprint
+    info, mult, donor = s.branch(float(w.schedule[nb - 1]), t, want_maps=True)
+    assert mult.sum() == w.W and info.n_recipients == (mult == 0).sum() == np.maximum(mult - 1, 0).sum()
+    rec = np.where(donor >= 0)[0]
+    assert rec.size > 0 and (mult[donor[rec]] >= 2).all() and (np.diff(donor[rec]) >= 0).all()
+    a1, c1 = s.get()
+    pick = rec[:: max(1, rec.size // 64)][:64]
+    np.testing.assert_array_equal(a1[pick], t * a0[donor[pick]] + (1.0 - t) * a0[pick])
+    keep = np.where(donor < 0)[0]
+    np.testing.assert_array_equal(a1[keep[:256]], a0[keep[:256]])
+    np.testing.assert_array_equal(c1[keep], c0[keep])
+    del a0
+    # one traced sweep of a contiguous window that holds recipients
+    lo = int(rec[rec.size // 2]) - 8
+    lo = max(0, min(lo, w.W - 16))
+    hi = lo + 16
+    _, _, y_g = s.stats()
+    o = _oracle(w, hi - lo, spectra=a1[lo:hi])
+    np.testing.assert_allclose(o.chi2, c1[lo:hi], rtol=1e-6)
+    o.chi2[:] = c1[lo:hi]
+    o.y[:] = y_g[lo:hi]
+    T = w.schedule[nb:nb + 1]
+    tg, _ = s.anneal(T, w.eta, trace_walkers=(lo, hi))
+    tr_o = np.zeros((hi - lo, 1, w.n_omega), dtype=oracle.TRACE_DTYPE)
+    for i in range(hi - lo):
+        for m in range(w.n_omega):
+            tr_o[i, 0, m] = _oracle_move(o, i, lo + i, nb, m, T[0])
+    assert compare_traces(tg, tr_o, T, w.A / w.n_omega) == 0
+    a2, c2 = s.get()
+    np.testing.assert_allclose(a2[lo:hi], o.a, rtol=0, atol=1e-10 * o.a.max())
+    np.testing.assert_allclose(c2[lo:hi], o.chi2, rtol=1e-9, atol=1e-14 * float(c1.max()))
+    s.close()
