@@ -278,7 +278,7 @@ def main_ours(args):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": {"workload": f"{w.name} (BASELINE.json configs[1]): N_omega={w.n_omega}, N_tau={w.n_tau}, W={w.W}, "
+                "config": {"workload": f"{w.name} (BASELINE.json configs[{['tiny', 'small', 'branching', 'noise', 'stress'].index(w.name)}]): N_omega={w.n_omega}, N_tau={w.n_tau}, W={w.W}, "
                                        f"sweeps={w.n_sweeps}, T {w.t0}->{w.t1} geometric, eps={w.eps}",
                            "step": "one whole anneal (all sweeps + final sail_get), walkers re-initialised untimed",
                            "parallelism": f"{world} independent replica(s), one per GPU", "l2": "flushed between steps (256 MiB write)",
