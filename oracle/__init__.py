@@ -68,6 +68,14 @@ def num_threads() -> int:
     return int(lib().orc_num_threads())
 
 
+def stencil(a, s):
+    """Eq. 27-29 on one spectrum (no renormalisation)."""
+    a = _f64(a)
+    out = np.empty_like(a)
+    lib().orc_stencil(C.c_int(a.size), C.c_double(s), _p(a), _p(out))
+    return out
+
+
 def philox4x32_10(ctr, key):
     c = np.asarray(ctr, dtype=np.uint32)
     k = np.asarray(key, dtype=np.uint32)
@@ -149,6 +157,10 @@ class Oracle:
 
     def resync(self):
         lib().orc_resync(C.byref(self.P), C.c_int64(self.W), _p(self.a), _p(self.M), _p(self.chi2))
+
+    def smooth(self, s):
+        """Eq. 27-29 + renormalisation of the second sum rule (reading S2) + resync, all walkers."""
+        lib().orc_smooth(C.byref(self.P), C.c_int64(self.W), C.c_double(s), _p(self.a), _p(self.M), _p(self.chi2))
 
     # --- sail_anneal -------------------------------------------------------------------
     def anneal(self, T_sched, resync_every=0, trace_walkers=None, want_flags=False):

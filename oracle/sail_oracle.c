@@ -22,6 +22,9 @@
  *                       vs from-scratch chi^2, Metropolis frequency exp(-D/T), T->0 / T->inf
  *   orc_amp_factor      Eq. 30 special values (y = a^2 for p=1, m=2)
  *   orc_branch          sum m = W, E[m] = w, t=1 copy / t=0 no-op, A,B preserved
+ *   orc_stencil         cosine (DCT-II) modes are eigenvectors with eigenvalue 1 - 2s(1 - cos(pi n/N));
+ *                       sum a kept, sum a w^m shifted by s domega (a_0 - a_{N-1}); s = 0 identity
+ *   orc_smooth          A, B restored to 1e-13, positivity; the choice of renormalisation (S2) is unpinned
  * Parity unpinned (paper silent; inputs identical on both sides): the width/shape of the
  * random move rho (eta, uniform), y_min, the acceptance window of Eq. 30, the comb choice of xi.
  */
@@ -404,6 +407,49 @@ int64_t orc_branch(const orc_problem *P, int64_t W, double *a, double *M, double
         chi2[i] = orc_chi2(n_tau, M + (size_t)i * n_tau, P->F, P->sigma);
     }
     return n_rec;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O9  smoothing, Eq. 27-29, SURVEY 8(f) row f3.
+ *   Eq. 27: a_j <- s a_{j-1} + (1 - 2s) a_j + s a_{j+1},  0 < j < N-1
+ *   Eq. 28: a_0 <- (1 - s) a_0 + s a_1          Eq. 29: a_{N-1} <- (1 - s) a_{N-1} + s a_{N-2}
+ * Reading S1: the stencil is applied to all bins simultaneously (every right-hand side is the OLD
+ * spectrum), terms added in the order written.  orc_stencil is exactly this and nothing else.
+ * The stencil keeps sum a (Eq. 12) and shifts sum a w^m (Eq. 14) by s domega (a_0 - a_{N-1}); the
+ * paper asks for "an additional renormalization" (:197) without saying which.  Reading S2:
+ * multiply by a linear tilt about the new mean frequency,
+ *      a_k <- a_k (1 + kappa (w^m_k - wbar)),  wbar = B'/A',  kappa = (B - B') / sum_k a_k (w^m_k - wbar)^2,
+ * which leaves A' untouched, restores B and, kappa being O(s / N), keeps every coefficient positive.
+ * (B is the problem's second sum, P->B.)  Afterwards the model and residue are recomputed (O7).
+ * ------------------------------------------------------------------------------------- */
+void orc_stencil(int n, double s, const double *a, double *out)
+{
+    const double c = 1.0 - 2.0 * s, e = 1.0 - s;
+    if (n == 1) { out[0] = a[0]; return; }
+    out[0] = e * a[0] + s * a[1];
+    for (int j = 1; j < n - 1; ++j) out[j] = (s * a[j - 1] + c * a[j]) + s * a[j + 1];
+    out[n - 1] = e * a[n - 1] + s * a[n - 2];
+}
+
+void orc_smooth(const orc_problem *P, int64_t W, double s, double *a, double *M, double *chi2)
+{
+    const int n = P->n_omega;
+    const double half = 0.5 * orc_domega(n, P->omega);
+    #pragma omp parallel for schedule(static)
+    for (int64_t w = 0; w < W; ++w) {
+        double *row = a + (size_t)w * n;
+        double *tmp = (double *)malloc((size_t)n * sizeof(double));
+        orc_stencil(n, s, row, tmp);
+        double A1 = 0.0, B1 = 0.0, V = 0.0;
+        for (int k = 0; k < n; ++k) { A1 += tmp[k]; B1 += tmp[k] * (P->omega[k] + half); }
+        const double wbar = B1 / A1;
+        for (int k = 0; k < n; ++k) { const double dw = (P->omega[k] + half) - wbar; V += tmp[k] * dw * dw; }
+        const double kappa = (V > 0.0) ? (P->B - B1) / V : 0.0;
+        for (int k = 0; k < n; ++k) row[k] = tmp[k] * (1.0 + kappa * ((P->omega[k] + half) - wbar));
+        free(tmp);
+        orc_forward(n, P->n_tau, P->K, row, M + (size_t)w * P->n_tau);
+        chi2[w] = orc_chi2(P->n_tau, M + (size_t)w * P->n_tau, P->F, P->sigma);
+    }
 }
 
 /* number of OpenMP threads the driver will use (reported as cpu_baseline.cores) */

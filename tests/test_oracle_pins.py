@@ -461,3 +461,66 @@ def test_oracle_reproduces_its_committed_trace():
             assert float(t[name]) == pytest.approx(float(val), rel=1e-11, abs=1e-300), name
         n += 1
     assert n == 96
+
+
+# ---- O9 smoothing, Eq. 27-29 ------------------------------------------------------
+def test_stencil_cosine_modes_are_eigenvectors():
+    """Eq. 27-29 is the 3-point diffusion stencil with reflecting ends: the DCT-II modes cos(pi n (j + 1/2) / N) are
+    its eigenvectors with eigenvalue 1 - 2 s (1 - cos(pi n / N)) (a textbook fact, not the oracle's own formula)."""
+    N, s = 48, 0.037
+    j = np.arange(N)
+    for n in (0, 1, 5, 17, N - 1):
+        mode = np.cos(np.pi * n * (j + 0.5) / N)
+        lam = 1.0 - 2.0 * s * (1.0 - math.cos(math.pi * n / N))
+        np.testing.assert_allclose(oracle.stencil(mode, s), lam * mode, rtol=0, atol=2e-15)
+
+
+def test_stencil_is_not_transposed_or_shifted_and_s0_is_identity():
+    """A single spike spreads s to each neighbour (and keeps 1 - s at an end bin); s = 0 changes nothing."""
+    N, s = 9, 0.25
+    for k in range(N):
+        e = np.zeros(N); e[k] = 1.0
+        want = np.zeros(N)
+        want[k] = 1 - 2 * s if 0 < k < N - 1 else 1 - s
+        if k > 0: want[k - 1] = s
+        if k < N - 1: want[k + 1] = s
+        np.testing.assert_allclose(oracle.stencil(e, s), want, rtol=0, atol=1e-16)
+    a = np.random.default_rng(3).random(N)
+    np.testing.assert_array_equal(oracle.stencil(a, 0.0), a)
+    ramp = np.arange(N, dtype=float)
+    np.testing.assert_allclose(oracle.stencil(ramp, s)[1:-1], ramp[1:-1], rtol=1e-15)   # interior of a linear ramp
+
+
+def test_stencil_keeps_first_sum_rule_and_shifts_the_second_as_the_paper_says():
+    """:197 — the first sum rule is preserved, the second violated 'of the order of s (a_{N-1} - a_0) / N': exactly
+    sum_j w_j (a'_j - a_j) = s domega (a_0 - a_{N-1}) for bin midpoints w_j (summation by parts)."""
+    rng = np.random.default_rng(5)
+    N, s, dw = 64, 0.03, 0.125
+    wm = (np.arange(N) + 0.5) * dw
+    for _ in range(5):
+        a = rng.random(N) + 0.01
+        b = oracle.stencil(a, s)
+        assert abs(b.sum() - a.sum()) <= 1e-14 * a.sum()
+        assert abs(((b - a) * wm).sum() - s * dw * (a[0] - a[-1])) <= 1e-13 * (a * wm).sum()
+
+
+def test_smooth_restores_both_sum_rules_keeps_positivity_and_resyncs(tiny):
+    """Reading S2 (linear tilt about the mean frequency) + resync: A and B back to 1e-13, a > 0, M = forward(a)."""
+    o = _oracle_for(tiny)
+    o.init_walkers(16)
+    o.anneal(tiny.schedule[:5])
+    a0 = o.a.copy()
+    wm = tiny.omega + 0.5 * tiny.domega
+    o.smooth(0.02)
+    np.testing.assert_allclose(o.a.sum(axis=1), tiny.A, rtol=1e-13)
+    np.testing.assert_allclose((o.a * wm).sum(axis=1), tiny.B, rtol=1e-13)
+    assert (o.a > 0).all()
+    st = np.array([oracle.stencil(r, 0.02) for r in a0])
+    assert np.abs(o.a / st - 1.0).max() < 1e-3                      # the renormalisation is a small correction
+    M, c2 = o.M.copy(), o.chi2.copy()
+    o.resync()
+    np.testing.assert_array_equal(o.M, M)
+    np.testing.assert_array_equal(o.chi2, c2)
+    o2 = _oracle_for(tiny); o2.init_walkers(16, a0)
+    o2.smooth(0.0)                                                   # s = 0: only rounding-level renormalisation
+    np.testing.assert_allclose(o2.a, a0, rtol=1e-12)
