@@ -335,6 +335,15 @@ def extra_workloads(torch, Sail, dev_index, peaks):
     flops = 2.0 * w.W * w.n_omega * w.n_tau
     out["stress_resync"] = {"seconds": t_rs, "tflops_fp64": flops / t_rs / 1e12,
                             "frac_of_fp64_alu_peak": flops / 2 / t_rs / peak}
+    # f3 smoothing (Eq. 27-29): stencil + renormalisation kernel (HBM bound: the spectra once in, once out), then a resync
+    s.smooth(0.02)
+    t_sm = timed(lambda: s.smooth(0.02))
+    sm_bytes = 16.0 * w.W * w.n_omega
+    t_st = max(t_sm - t_rs, 1e-9)
+    out["stress_smooth"] = {"seconds": t_sm, "stencil_seconds": t_st, "algorithmic_GB": sm_bytes / 1e9,
+                            "stencil_GBps": sm_bytes / t_st / 1e9,
+                            "frac_of_measured_hbm": sm_bytes / t_st / 1e9 / peaks.get("hbm_gbs", 6553.3),
+                            "note": "stencil time = whole call minus the resync time measured above"}
     # one branching event per imprint strength, each on a fresh population (init + 1 sweep) so that the recipient
     # count belongs to the timed event itself; the kernels are warmed up on the old population first
     _, c2 = s.get(spectra=False)

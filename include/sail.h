@@ -156,6 +156,15 @@ SAIL_API int sail_branch(sail_t *h, double T, double t_imprint, sail_branch_info
 SAIL_API int sail_resync(sail_t *h);
 
 /*
+ * sail_smooth — the smoothing step between blocks (Eq. 27-29): every walker's spectrum goes through
+ * the three-point stencil a_j <- s a_{j-1} + (1 - 2s) a_j + s a_{j+1} (reflecting end bins, all bins at once), the
+ * second sum rule the stencil violates (:197) is restored by a linear tilt about the mean frequency (DESIGN.md
+ * reading S2), then model and residue are recomputed as in sail_resync.  0 <= s <= 0.5 (the paper uses a few
+ * percent); n_omega <= 2048.  Asynchronous on the stream.
+ */
+SAIL_API int sail_smooth(sail_t *h, double s);
+
+/*
  * sail_get — copy results out.  spectra [W][n_omega] (true coefficients a_k), chi2 [W]; either may
  * be NULL.  on_device = 0: HOST destinations (synchronises); 1: DEVICE destinations (stream-ordered).
  */

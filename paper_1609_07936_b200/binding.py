@@ -18,7 +18,7 @@ SAIL_OK, SAIL_ERR_ARG, SAIL_ERR_GRID, SAIL_ERR_ALLOC, SAIL_ERR_CUDA, SAIL_ERR_ST
 
 EXPORTS = ["sail_workspace_bytes", "sail_create", "sail_init_walkers", "sail_anneal", "sail_branch",
            "sail_resync", "sail_get", "sail_get_model", "sail_stats", "sail_set_walkers", "sail_set_sweep",
-           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak", "sail_microbench"]
+           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak", "sail_microbench", "sail_smooth"]
 
 
 class SailError(RuntimeError):
@@ -67,6 +67,7 @@ def lib():
         L.sail_anneal.argtypes = [C.c_void_p, C.c_void_p, C.c_int64, C.POINTER(sail_anneal_params)]
         L.sail_branch.argtypes = [C.c_void_p, C.c_double, C.c_double, C.POINTER(sail_branch_info), C.c_void_p, C.c_void_p]
         L.sail_resync.argtypes = [C.c_void_p]
+        L.sail_smooth.argtypes = [C.c_void_p, C.c_double]
         L.sail_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32]
         L.sail_get_model.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
         L.sail_stats.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -199,6 +200,10 @@ class Sail:
 
     def resync(self):
         self._check(self._L.sail_resync(self._h))
+
+    def smooth(self, s):
+        """Eq. 27-29 + renormalisation of the second sum rule + resync (include/sail.h: sail_smooth)."""
+        self._check(self._L.sail_smooth(self._h, C.c_double(s)))
 
     def get(self, spectra=True, chi2=True):
         sp = np.empty((self.W, self.n_omega)) if spectra else None

@@ -330,6 +330,15 @@ int sail_resync(sail_t *h)
     return launch_forward(h, 0, h->W);
 }
 
+int sail_smooth(sail_t *h, double s)
+{
+    if (!h) return SAIL_ERR_ARG;
+    if (!h->initialised) return set_err(h, SAIL_ERR_STATE, "sail_smooth before sail_init_walkers");
+    if (!(s >= 0.0 && s <= 0.5)) return set_err(h, SAIL_ERR_ARG, "smoothing amplitude s must lie in [0, 0.5] (got %g)", s);
+    SAIL_CUDA_OK(h, cudaSetDevice(h->device));
+    return launch_smooth(h, s);
+}
+
 int sail_get(sail_t *h, double *spectra, double *chi2, int32_t on_device)
 {
     if (!h) return SAIL_ERR_ARG;

@@ -474,3 +474,36 @@ def test_branching_and_noise_configurations_sampled_parity(name):
     np.testing.assert_allclose(a2[lo:hi], o.a, rtol=0, atol=1e-10 * o.a.max())
     np.testing.assert_allclose(c2[lo:hi], o.chi2, rtol=1e-9, atol=1e-14 * float(c1.max()))
     s.close()
+
+
+@pytest.mark.parametrize("name,W,s_amp", [("tiny", 64, 0.02), ("small", 97, 0.05), ("stress", 19, 0.01), ("tiny", 5, 0.0)])
+def test_smoothing_parity(name, W, s_amp):
+    """f3 (Eq. 27-29 + reading S2 + resync): from the identical annealed state the smoothed spectra agree to rounding
+    of the three block sums (1e-13), both sum rules are restored, model and residue follow; then the chains continue
+    in lockstep (the smoothed state is a valid walker state)."""
+    w = wl.make(name, simpson_intervals=20_000)
+    o = _oracle(w, W)
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED, spectra=o.a)
+    T = wl.geometric_schedule(1.0, 0.5, 3)
+    s.anneal(T, w.eta)
+    o.anneal(T)
+    a0, c0 = s.get()
+    o.a[:] = a0; o.resync(); s.resync()                  # identical spectra, residues from scratch on both sides
+    s.smooth(s_amp); o.smooth(s_amp)
+    a1, c1 = s.get()
+    np.testing.assert_allclose(a1, o.a, rtol=1e-13, atol=1e-300)
+    np.testing.assert_allclose(s.get_model(), o.M, rtol=1e-11)
+    np.testing.assert_allclose(c1, o.chi2, rtol=1e-8)
+    wm = w.omega + 0.5 * w.domega
+    np.testing.assert_allclose(a1.sum(axis=1), w.A, rtol=1e-12)
+    np.testing.assert_allclose((a1 * wm).sum(axis=1), w.B, rtol=1e-12)
+    assert (a1 >= 0).all()
+    if s_amp == 0.0:
+        np.testing.assert_allclose(a1, a0, rtol=1e-12)
+    o.a[:] = a1; o.resync(); s.set_walkers(0, a1)
+    T2 = wl.geometric_schedule(0.5, 0.3, 2)
+    tg, fg = s.anneal(T2, w.eta, trace_walkers=(0, W), want_flags=True)
+    to, fo = o.anneal(T2, trace_walkers=(0, W), want_flags=True)
+    assert compare_traces(tg, to, T2, w.A / w.n_omega) == 0
+    s.close()
