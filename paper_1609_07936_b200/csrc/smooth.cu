@@ -2,7 +2,8 @@
 //   Eq. 27: a_j <- s a_{j-1} + (1 - 2s) a_j + s a_{j+1}     Eq. 28-29: reflecting end bins
 // applied to all bins simultaneously (S1), followed by the renormalisation of the second sum rule (S2): a linear
 // tilt a_k (1 + kappa (w^m_k - wbar)) about the new mean frequency, kappa = (B - B') / sum a_k (w^m_k - wbar)^2.
-// One 128-thread CTA per walker row: the row is read once (coalesced, staged in shared memory for the neighbour taps), three
+// One 128-thread CTA per walker row: the row is read once (cp.async into a double-buffered shared-memory stage that
+// serves the neighbour taps; the next row streams in while this one is reduced), three
 // block sums (A', B', then the variance), written once: 16 N_omega bytes of HBM traffic per walker.  The model and
 // the residue are then refreshed by the dense forward kernel (row A7).
 #include "sail_internal.cuh"
@@ -32,14 +33,31 @@ constexpr int kSmoothPerThread = 16;                   // 128 threads x 16 = row
 __global__ void __launch_bounds__(kSmoothThreads) smooth_kernel(int n_omega, long long W, double s, double B, double domega,
                                                      const double *__restrict__ omega, double *__restrict__ a)
 {
-    extern __shared__ double row[];                    // [n_omega] old spectrum
+    extern __shared__ __align__(16) double rows[];     // [2][n_omega rounded up to even]: old spectra, double-buffered
     __shared__ double red[4 * (kSmoothThreads / 32)];
     const double c = 1.0 - 2.0 * s, e = 1.0 - s, half = 0.5 * domega;
     const int nwarps = blockDim.x >> 5;
-    for (long long w = blockIdx.x; w < W; w += gridDim.x) {
+    const int n_pad = (n_omega + 1) & ~1;
+    const bool vec = (n_omega & 1) == 0;               // rows are 16-byte aligned: cp.async of pairs
+    // the next row of this CTA streams into the other buffer (cp.async) while the current one is reduced
+    auto prefetch = [&](long long w, int buf) {
+        if (vec && w < W) {
+            const uint32_t dst = (uint32_t)__cvta_generic_to_shared(rows + buf * n_pad);
+            const double *src = a + (size_t)w * n_omega;
+            for (int k2 = threadIdx.x; k2 < n_omega / 2; k2 += blockDim.x)
+                asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" :: "r"(dst + (uint32_t)k2 * 16u), "l"(src + 2 * k2) : "memory");
+        }
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    prefetch(blockIdx.x, 0);
+    int it = 0;
+    for (long long w = blockIdx.x; w < W; w += gridDim.x, ++it) {
         double *aw = a + (size_t)w * n_omega;
-        __syncthreads();                               // the previous row (and its sums) are no longer read
-        for (int k = threadIdx.x; k < n_omega; k += blockDim.x) row[k] = aw[k];
+        double *row = rows + (it & 1) * n_pad;
+        prefetch(w + gridDim.x, (it & 1) ^ 1);         // its previous contents were last read before the barriers of row it-1
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+        if (!vec)
+            for (int k = threadIdx.x; k < n_omega; k += blockDim.x) row[k] = aw[k];
         __syncthreads();
         double nv[kSmoothPerThread];
         double sA = 0.0, sB = 0.0;
@@ -84,7 +102,7 @@ int launch_smooth(sail_handle *h, double s)
         return set_err(h, SAIL_ERR_ARG, "sail_smooth supports n_omega <= %d", kSmoothThreads * kSmoothPerThread);
     const long long W = h->W;
     const int blocks = (int)(W < (long long)h->num_sms * 12 ? W : (long long)h->num_sms * 12);
-    smooth_kernel<<<blocks, kSmoothThreads, (size_t)h->n_omega * sizeof(double), h->stream>>>(h->n_omega, W, s, h->B, h->domega,
+    smooth_kernel<<<blocks, kSmoothThreads, (size_t)2 * ((h->n_omega + 1) & ~1) * sizeof(double), h->stream>>>(h->n_omega, W, s, h->B, h->domega,
                                                                                  h->tab.omega, h->st.a);
     SAIL_LAUNCH_OK(h, "smooth_kernel");
     return launch_forward(h, 0, W);
