@@ -107,6 +107,25 @@ __device__ __forceinline__ double warp_sum_dmma(double x)
     return t0;
 }
 
+// The same for groups of G = 8, 16 or 32 consecutive lanes (every lane gets the sum over ITS group): after the first
+// product and the pair sum, h held by a lane with lane % 4 = q is the sum over lanes 8q .. 8q+7; the second product
+// takes A[m][k] = 1 where octet k belongs to the group of row m (m = lane / 4 is the row a lane reads back).
+template <int G>
+__device__ __forceinline__ double group_sum_dmma(double x)
+{
+    const int lane = threadIdx.x & 31;
+    const int m = lane >> 2, k = lane & 3;
+    const double sel = (G == 32) ? 1.0 : (G == 16) ? (((k < 2) == (m < 4)) ? 1.0 : 0.0) : ((k == (m >> 1)) ? 1.0 : 0.0);
+    double c0, c1, t0, t1;
+    const double one = 1.0, zero = 0.0;
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%4,%4};"
+        : "=d"(c0), "=d"(c1) : "d"(one), "d"(x), "d"(zero));
+    const double h = c0 + c1;
+    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%4,%4};"
+        : "=d"(t0), "=d"(t1) : "d"(sel), "d"(h), "d"(zero));
+    return t0;
+}
+
 // Eq. 30: y from the sweep's acceptance rate
 __device__ __forceinline__ double amp_factor(const SweepArgs &P, int acc_sweep, double y)
 {

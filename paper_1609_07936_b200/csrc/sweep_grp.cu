@@ -159,8 +159,7 @@ sweep_kernel_grp(const SweepArgs P)
                         else       acc_a = fma(d[i], t, acc_a);
                     }
                     double dchi2 = (C > 1) ? acc_a + acc_b : acc_a;
-#pragma unroll
-                    for (int off = G / 2; off > 0; off >>= 1) dchi2 += __shfl_xor_sync(0xffffffffu, dchi2, off);
+                    dchi2 = group_sum_dmma<G>(dchi2);         // sum over this walker's G lanes, no shuffles
                     // ---- Metropolis (row A5, Eq. 10), per walker ---------------------------------------------------
                     const bool acc = active && (dchi2 < th.x);
                     const int ia = acc ? 1 : 0;
@@ -168,20 +167,21 @@ sweep_kernel_grp(const SweepArgs P)
                     if (TRACE) { if (active && sub == m) { tr_fl = 4 | (ia << 1); tr_dchi2 = dchi2; } }
                     mlast = active ? m : mlast;
                     if (__ballot_sync(0xffffffffu, acc)) {
+                        // a real branch: the accepting groups run the update once, together; the others wait
+                        if (acc) {
 #pragma unroll
-                        for (int i = 0; i < C; ++i) {
-                            add_if(mt[i], d[i], ia);
-                            if (W2REG) fma_if(G2[i], W2[i], d[i], ia);
-                            else       fma_if(G2[i], Wt[i], d[i] + d[i], ia);
+                            for (int i = 0; i < C; ++i) {
+                                mt[i] += d[i];
+                                if (W2REG) G2[i] = fma(W2[i], d[i], G2[i]);
+                                else       G2[i] = fma(Wt[i], d[i] + d[i], G2[i]);
+                            }
+                            chi2 += dchi2;
+                            g = fma(alpha, g, g);
+                            ginv *= th.y;
+                            // the lane that owns the accepted move holds its new coefficients from its last screen
+                            if (sub == m) { *my_pp = xp * ginv; *my_ps = xs * ginv; }
+                            acc_sweep++;
                         }
-                        add_if(chi2, dchi2, ia);
-                        fma_if(g, alpha, g, ia);
-                        mul_if(ginv, th.y, ia);
-                        // the lane that owns the accepted move holds its new coefficients from its last screen
-                        const int mine = (acc && sub == m) ? 1 : 0;
-                        stg_f64_if(my_pp, xp * ginv, mine);
-                        stg_f64_if(my_ps, xs * ginv, mine);
-                        acc_sweep += ia;
                         __syncwarp();
                         ball = screen();              // a spectrum changed: screen the pending moves again
                     } else {
