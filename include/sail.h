@@ -111,8 +111,7 @@ typedef struct {
     double  eta;             /* base amplitude: rho = 1 - y eta (2u - 1), requires 0 < eta < 1 (reading G6) */
     int32_t amp_mode;        /* 0: y = 1;  1: Eq. 30 from the previous sweep's acceptance  */
     int32_t lanes_per_walker;/* sweep-kernel form, a tuning knob (all forms make the same moves and decisions):
-                              * 0 auto = 32, or 16 where that pads N_tau less and W still fills the GPU;
-                              * 32 screened one-walker-per-warp kernel, DMMA warp sum;
+                              * 0 / 32 screened one-walker-per-warp kernel, DMMA warp sum (default);
                               * 37 the same with the shuffle butterfly; 35 the same, other register budget;
                               * 34 unscreened form; 8 / 16 lanes per walker: several walkers per warp in
                               * lockstep; 36 the 32-lane instance of that kernel          */

@@ -537,16 +537,9 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     const int req = p->lanes_per_walker;
     if (!(req == 0 || req == 8 || req == 16 || req == 32 || (req >= 34 && req <= 37)))
         return set_err(h, SAIL_ERR_ARG, "lanes_per_walker=%d is not one of 0, 8, 16, 32, 34..37", req);
-    int G = pick_lanes(req);
-    int auto16 = 0;
-    if (req == 0) {
-        // auto: 16 lanes per walker (two walkers per warp, sweep_grp.cu) when that pads the tau grid less than 32 lanes
-        // do (N_tau = 200: 208 slots instead of 224) AND the population still fills every SM with such warps; measured
-        // on Branching: 0.281 against 0.269 of the FP64 roofline (profiles/r01_sweep_variants.md)
-        const int C16 = (h->n_tau + 15) / 16, C32 = (h->n_tau + 31) / 32;
-        const int maxw16 = C16 <= 7 ? 16 : 12;
-        if (C16 * 16 < C32 * 32 && C16 <= 13 && (h->W + 1) / 2 >= (long long)h->num_sms * maxw16) { G = 16; auto16 = 1; }
-    }
+    const int G = pick_lanes(req);
+    // (16 lanes per walker win the first sweeps of Branching, 0.281 against 0.269, but lose over the whole anneal,
+    // 0.270 against 0.280: auto stays with one walker per warp)
     const int C = (h->n_tau + G - 1) / G;
     if (C > 16) return set_err(h, SAIL_ERR_ARG, "n_tau=%d needs more than 16 tau-points per lane at %d lanes", h->n_tau, G);
     int rc = ensure_sweep_tables(h, G);
@@ -576,7 +569,7 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     const bool trace = (p->trace != nullptr) || (p->flags != nullptr);
 
     // grouped screened kernel (sweep_grp.cu): 8 / 16 lanes per walker, 36 = its one-walker-per-warp instance
-    if (req == 8 || req == 16 || req == 36 || auto16) return launch_sweep_grp(h, a, G, C, trace, 0);
+    if (req == 8 || req == 16 || req == 36) return launch_sweep_grp(h, a, G, C, trace, 0);
 
 #define SAIL_VARIANT(CC, MW, MODE)                                                                                  \
     {                                                                                                                   \
