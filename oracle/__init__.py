@@ -68,6 +68,24 @@ def num_threads() -> int:
     return int(lib().orc_num_threads())
 
 
+def selfcool_temperature(b, chi2_0, chi2_ave, chi2_min, n_boil, n_ramp, T_start=10.0, freeze_rate=1.0):
+    """Self-cooling, temperature of block b = 0, 1, ... from the residues
+    the population has reached (chi2_ave, chi2_min: measured after block b-1), readings C1-C3 of DESIGN.md:
+      block 0            T = T_start * chi2_0          (unit of T = starting residue, T_start = 10, :216)
+      boil   (b <= n_boil)        T = chi2_ave         ("we set T close chi2_ave")
+      ramp   (next n_ramp blocks) T goes linearly from chi2_ave to chi2_min ("slowly ramped towards chi2_min")
+      freeze (afterwards)         T = chi2_min / (1 + freeze_rate * steps), steps = blocks since the ramp ended
+                                  ("lowered below the minimal residue ... proportionately to the number of steps")."""
+    if b == 0:
+        return T_start * chi2_0
+    if b <= n_boil:
+        return chi2_ave
+    if b <= n_boil + n_ramp:
+        f = (b - n_boil) / n_ramp
+        return chi2_ave + (chi2_min - chi2_ave) * f
+    return chi2_min / (1.0 + freeze_rate * (b - n_boil - n_ramp))
+
+
 def stencil(a, s):
     """Eq. 27-29 on one spectrum (no renormalisation)."""
     a = _f64(a)
@@ -157,6 +175,26 @@ class Oracle:
 
     def resync(self):
         lib().orc_resync(C.byref(self.P), C.c_int64(self.W), _p(self.a), _p(self.M), _p(self.chi2))
+
+    def anneal_selfcool(self, n_blocks, sweeps_per_block, n_boil, n_ramp, t_imprint=0.1, smooth_s=0.0,
+                        T_start=10.0, freeze_rate=1.0, T_override=None):
+        """The paper's block protocol (:218-220) with self-cooling: per block, T from the population's residues, then
+        sweeps_per_block sweeps at that T, smoothing (if smooth_s > 0), one branching event at 1/T.  T_override[b]
+        replaces the rule (used by the parity tests to drive both sides with the same temperatures).
+        Returns (T, chi2_ave, chi2_min) per block."""
+        chi2_0 = float(np.mean(self.chi2))
+        Ts, aves, mins = [], [], []
+        for b in range(n_blocks):
+            ave, mn = float(np.mean(self.chi2)), float(np.min(self.chi2))
+            T = selfcool_temperature(b, chi2_0, ave, mn, n_boil, n_ramp, T_start, freeze_rate)
+            if T_override is not None:
+                T = float(T_override[b])
+            Ts.append(T); aves.append(ave); mins.append(mn)
+            self.anneal(np.full(sweeps_per_block, T))
+            if smooth_s > 0.0:
+                self.smooth(smooth_s)
+            self.branch(T, t_imprint)
+        return np.array(Ts), np.array(aves), np.array(mins)
 
     def smooth(self, s):
         """Eq. 27-29 + renormalisation of the second sum rule (reading S2) + resync, all walkers."""

@@ -524,3 +524,34 @@ def test_smooth_restores_both_sum_rules_keeps_positivity_and_resyncs(tiny):
     o2 = _oracle_for(tiny); o2.init_walkers(16, a0)
     o2.smooth(0.0)                                                   # s = 0: only rounding-level renormalisation
     np.testing.assert_allclose(o2.a, a0, rtol=1e-12)
+
+
+# ---- f1 self-cooling ------------------------------------------------------------
+def test_selfcool_rule_follows_the_papers_statements():
+    """What the paper fixes: T starts at 10 starting residues (:216); it sits at chi2_ave while boiling, is ramped
+    towards chi2_min, then goes BELOW chi2_min and falls in proportion to the number of steps (:162).  The lengths
+    of the phases and the rate are the build's constants (readings C2: unpinned)."""
+    f = oracle.selfcool_temperature
+    chi0, ave, mn, nb, nr = 3.0e8, 5.0e4, 2.0e3, 3, 4
+    assert f(0, chi0, ave, mn, nb, nr) == 10.0 * chi0
+    assert all(f(b, chi0, ave, mn, nb, nr) == ave for b in (1, 2, 3))
+    ramp = [f(b, chi0, ave, mn, nb, nr) for b in range(nb + 1, nb + nr + 1)]
+    assert all(x > y for x, y in zip([ave] + ramp, ramp)) and ramp[-1] == mn and ave > ramp[0] > mn
+    np.testing.assert_allclose(np.diff(ramp), (mn - ave) / nr, rtol=1e-12)              # linear
+    fr = [f(b, chi0, ave, mn, nb, nr, freeze_rate=0.5) for b in range(nb + nr + 1, nb + nr + 6)]
+    assert all(x < mn for x in fr)
+    np.testing.assert_allclose([x * (1 + 0.5 * k) for k, x in enumerate(fr, start=1)], mn, rtol=1e-14)   # ~ 1 / steps
+
+
+def test_selfcool_protocol_runs_blocks_of_sweeps_branching_and_smoothing(tiny):
+    """The block protocol on a small population: temperatures are the rule applied to the residues BEFORE each block,
+    the sweep counter advances by the block length, sum rules survive smoothing + branching."""
+    o = _oracle_for(tiny); o.init_walkers(24)
+    c0 = float(np.mean(o.chi2))
+    T, ave, mn = o.anneal_selfcool(5, 4, n_boil=1, n_ramp=2, smooth_s=0.01)
+    assert T[0] == 10.0 * c0 and ave[0] == c0 and o.sweep == 20
+    for b in range(5):
+        assert T[b] == oracle.selfcool_temperature(b, c0, ave[b], mn[b], 1, 2)
+    wm = tiny.omega + 0.5 * tiny.domega
+    np.testing.assert_allclose(o.a.sum(axis=1), tiny.A, rtol=1e-11)
+    np.testing.assert_allclose((o.a * wm).sum(axis=1), tiny.B, rtol=1e-11)
