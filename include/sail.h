@@ -165,6 +165,37 @@ SAIL_API int sail_resync(sail_t *h);
 SAIL_API int sail_smooth(sail_t *h, double s);
 
 /*
+ * sail_chi2_stats — the two population statistics the self-cooling schedule feeds on: the smallest
+ * and the mean residue over the W walkers, HOST outputs (either may be NULL).  Fixed summation order: bit-reproducible.
+ * Synchronises the stream.
+ */
+SAIL_API int sail_chi2_stats(sail_t *h, double *chi2_min, double *chi2_mean);
+
+/* Parameters of sail_anneal_selfcool (readings C1-C3; the paper gives no constants beyond T_start). */
+typedef struct {
+    int32_t sweeps_per_block;   /* k of "each block consists of some k N_omega steps" (paper: 100, :218)          */
+    int32_t n_boil, n_ramp;     /* blocks at T = chi2_ave, then blocks of the linear ramp to chi2_min (n_ramp >= 1) */
+    double  T_start;            /* temperature of block 0 in units of the starting residue (paper: 10, :216)        */
+    double  freeze_rate;        /* freeze-out: T = chi2_min / (1 + freeze_rate * blocks since the ramp ended)       */
+    double  t_imprint;          /* imprint strength of the branching after every block (paper: 0.1, :220)          */
+    double  smooth_s;           /* smoothing amplitude applied before the branching; 0 = no smoothing (:190)        */
+    int32_t branch;             /* 0: no branching                                                                  */
+    int32_t reserved;
+    const double *T_override;   /* HOST [n_blocks] or NULL: use these temperatures instead of the rule (tests)      */
+    sail_anneal_params anneal;  /* eta, Eq. 30 parameters, kernel form, traces for the sweeps of the blocks         */
+} sail_selfcool_params;
+
+/*
+ * sail_anneal_selfcool — n_blocks blocks of the paper's protocol (:218-220) with the self-cooling schedule of
+ * section 2.4 (:160-162): before each block the residues chi2_ave, chi2_min are measured (sail_chi2_stats), the block's
+ * temperature follows from them (block 0: T_start starting residues; boil: chi2_ave; ramp: linear to chi2_min; freeze-out:
+ * below chi2_min, ~ 1 / blocks), then sweeps_per_block sweeps at that temperature, sail_smooth (if smooth_s > 0) and
+ * one sail_branch at 1/T.  T_out, chi2_ave_out, chi2_min_out: HOST [n_blocks] or NULL.  Synchronises once per block.
+ */
+SAIL_API int sail_anneal_selfcool(sail_t *h, const sail_selfcool_params *p, int64_t n_blocks, double *T_out,
+                                  double *chi2_ave_out, double *chi2_min_out);
+
+/*
  * sail_get — copy results out.  spectra [W][n_omega] (true coefficients a_k), chi2 [W]; either may
  * be NULL.  on_device = 0: HOST destinations (synchronises); 1: DEVICE destinations (stream-ordered).
  */

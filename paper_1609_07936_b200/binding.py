@@ -18,7 +18,7 @@ SAIL_OK, SAIL_ERR_ARG, SAIL_ERR_GRID, SAIL_ERR_ALLOC, SAIL_ERR_CUDA, SAIL_ERR_ST
 
 EXPORTS = ["sail_workspace_bytes", "sail_create", "sail_init_walkers", "sail_anneal", "sail_branch",
            "sail_resync", "sail_get", "sail_get_model", "sail_stats", "sail_set_walkers", "sail_set_sweep",
-           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak", "sail_microbench", "sail_smooth"]
+           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak", "sail_microbench", "sail_smooth", "sail_chi2_stats", "sail_anneal_selfcool"]
 
 
 class SailError(RuntimeError):
@@ -37,6 +37,13 @@ class sail_anneal_params(C.Structure):
                 ("amp_p", C.c_double), ("amp_m", C.c_double), ("y_min", C.c_double),
                 ("resync_every", C.c_int64), ("trace_lo", C.c_int64), ("trace_hi", C.c_int64),
                 ("trace", C.c_void_p), ("flags", C.c_void_p)]
+
+
+class sail_selfcool_params(C.Structure):
+    _fields_ = [("sweeps_per_block", C.c_int32), ("n_boil", C.c_int32), ("n_ramp", C.c_int32),
+                ("T_start", C.c_double), ("freeze_rate", C.c_double), ("t_imprint", C.c_double),
+                ("smooth_s", C.c_double), ("branch", C.c_int32), ("reserved", C.c_int32),
+                ("T_override", C.c_void_p), ("anneal", sail_anneal_params)]
 
 
 class sail_branch_info(C.Structure):
@@ -68,6 +75,9 @@ def lib():
         L.sail_branch.argtypes = [C.c_void_p, C.c_double, C.c_double, C.POINTER(sail_branch_info), C.c_void_p, C.c_void_p]
         L.sail_resync.argtypes = [C.c_void_p]
         L.sail_smooth.argtypes = [C.c_void_p, C.c_double]
+        L.sail_chi2_stats.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.sail_anneal_selfcool.argtypes = [C.c_void_p, C.POINTER(sail_selfcool_params), C.c_int64, C.c_void_p,
+                                           C.c_void_p, C.c_void_p]
         L.sail_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32]
         L.sail_get_model.argtypes = [C.c_void_p, C.c_void_p, C.c_int32]
         L.sail_stats.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
@@ -187,6 +197,28 @@ class Sail:
         if flags_t is not None:
             flags = flags_t.cpu().numpy().reshape(self.W, T.size, self.n_omega)
         return trace, flags
+
+    def chi2_stats(self):
+        """(min, mean) of chi^2 over the population (include/sail.h: sail_chi2_stats)."""
+        mn, mean = C.c_double(), C.c_double()
+        self._check(self._L.sail_chi2_stats(self._h, C.byref(mn), C.byref(mean)))
+        return mn.value, mean.value
+
+    def anneal_selfcool(self, n_blocks, sweeps_per_block, n_boil, n_ramp, eta, t_imprint=0.1, smooth_s=0.0, T_start=10.0,
+                        freeze_rate=1.0, branch=True, T_override=None, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6,
+                        lanes_per_walker=0):
+        """The paper's block protocol with self-cooling (include/sail.h: sail_anneal_selfcool).
+        Returns (T, chi2_ave, chi2_min), one entry per block."""
+        p = sail_selfcool_params()
+        p.sweeps_per_block, p.n_boil, p.n_ramp = sweeps_per_block, n_boil, n_ramp
+        p.T_start, p.freeze_rate, p.t_imprint, p.smooth_s, p.branch = T_start, freeze_rate, t_imprint, smooth_s, int(branch)
+        ov = _f64(T_override) if T_override is not None else None
+        p.T_override = ov.ctypes.data if ov is not None else None
+        p.anneal.eta, p.anneal.amp_mode, p.anneal.lanes_per_walker = eta, amp_mode, lanes_per_walker
+        p.anneal.amp_p, p.anneal.amp_m, p.anneal.y_min = amp_p, amp_m, y_min
+        T, ave, mn = np.zeros(n_blocks), np.zeros(n_blocks), np.zeros(n_blocks)
+        self._check(self._L.sail_anneal_selfcool(self._h, C.byref(p), n_blocks, _ptr(T), _ptr(ave), _ptr(mn)))
+        return T, ave, mn
 
     def branch(self, T, t_imprint, want_maps=False):
         info = sail_branch_info()

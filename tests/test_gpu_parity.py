@@ -507,3 +507,35 @@ def test_smoothing_parity(name, W, s_amp):
     to, fo = o.anneal(T2, trace_walkers=(0, W), want_flags=True)
     assert compare_traces(tg, to, T2, w.A / w.n_omega) == 0
     s.close()
+
+
+def test_selfcool_protocol_parity():
+    """f1 (self-cooling, :160-162, :216-220): (i) sail_chi2_stats against numpy; (ii) the library's rule gives the
+    oracle's temperatures from the library's own residues; (iii) driven with the SAME temperatures, the whole block
+    protocol (sweeps + smoothing + branching, 6 blocks) leaves both sides in the same state."""
+    w = wl.make("tiny", simpson_intervals=20_000)
+    W, nb, k, n_boil, n_ramp = 64, 6, 4, 1, 2
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED)
+    s.anneal(np.full(2, 1e6), w.eta)
+    _, c2 = s.get()
+    mn, mean = s.chi2_stats()
+    assert mn == c2.min() and abs(mean - c2.mean()) <= 1e-13 * c2.mean()
+    s.init_walkers(W, w.A, w.B, SEED)
+    T, ave, mins = s.anneal_selfcool(nb, k, n_boil, n_ramp, w.eta, t_imprint=0.1, smooth_s=0.01)
+    for b in range(nb):
+        want = oracle.selfcool_temperature(b, ave[0], ave[b], mins[b], n_boil, n_ramp)
+        assert abs(T[b] - want) <= 1e-14 * want
+    assert T[0] == 10.0 * ave[0] and (np.diff(T[n_boil:]) < 0).all() and T[-1] < mins[-1]
+    o = _oracle(w, W)
+    To, aveo, mino = o.anneal_selfcool(nb, k, n_boil, n_ramp, t_imprint=0.1, smooth_s=0.01, T_override=T)
+    np.testing.assert_allclose(aveo, ave, rtol=1e-8)
+    np.testing.assert_allclose(mino, mins, rtol=1e-8)
+    a, c2 = s.get()
+    np.testing.assert_allclose(a, o.a, rtol=0, atol=1e-9 * o.a.max())
+    np.testing.assert_allclose(c2, o.chi2, rtol=1e-7)
+    # the oracle's OWN schedule (its rule on its residues) is the same to the accuracy of the residues
+    o2 = _oracle(w, W)
+    T2, _, _ = o2.anneal_selfcool(nb, k, n_boil, n_ramp, t_imprint=0.1, smooth_s=0.01)
+    np.testing.assert_allclose(T2[:3], T[:3], rtol=1e-8)
+    s.close()
