@@ -53,6 +53,7 @@ def lib():
         _lib.orc_amp_factor.argtypes = [C.c_double] * 4
         _lib.orc_branch.restype = C.c_int64
         _lib.orc_num_threads.restype = C.c_int
+        _lib.orc_branch_zeros.restype = C.c_int64
     return _lib
 
 
@@ -172,6 +173,21 @@ class Oracle:
         self.feas = np.zeros(W, dtype=np.int64)
         self.sweep = 0
         self.resync()
+
+    def branch_zeros(self, T):
+        """Number of zero multipliers the comb of O8 gives at temperature T (state untouched)."""
+        return int(lib().orc_branch_zeros(C.byref(self.P), C.c_int64(self.W), _p(self.chi2), C.c_double(T), C.c_int64(self.sweep)))
+
+    def branch_fraction(self, fraction, t_imprint):
+        """f2: find 1/T so that `fraction` of the walkers get multiplier zero (reading B6), then branch at that T.
+        Returns (T, n_recipients, mult, donor); T = 0 means no event (degenerate population)."""
+        T = C.c_double(0.0)
+        ok = lib().orc_branch_fraction_T(C.byref(self.P), C.c_int64(self.W), _p(self.chi2), C.c_double(fraction),
+                                         C.c_int64(self.sweep), C.byref(T))
+        if not ok:
+            return 0.0, 0, None, None
+        n_rec, mult, donor = self.branch(T.value, t_imprint)
+        return T.value, n_rec, mult, donor
 
     def resync(self):
         lib().orc_resync(C.byref(self.P), C.c_int64(self.W), _p(self.a), _p(self.M), _p(self.chi2))

@@ -22,6 +22,8 @@
  *                       vs from-scratch chi^2, Metropolis frequency exp(-D/T), T->0 / T->inf
  *   orc_amp_factor      Eq. 30 special values (y = a^2 for p=1, m=2)
  *   orc_branch          sum m = W, E[m] = w, t=1 copy / t=0 no-op, A,B preserved
+ *   orc_branch_fraction_T  zeros(T) = 0 as T -> inf and grows as T falls; the T found brackets the target count
+ *                       (zeros(T) >= n0 > zeros(T (1 + 1e-9))); the bracketing path itself (B6) is unpinned
  *   orc_stencil         cosine (DCT-II) modes are eigenvectors with eigenvalue 1 - 2s(1 - cos(pi n/N));
  *                       sum a kept, sum a w^m shifted by s domega (a_0 - a_{N-1}); s = 0 identity
  *   orc_smooth          A, B restored to 1e-13, positivity; the choice of renormalisation (S2) is unpinned
@@ -407,6 +409,70 @@ int64_t orc_branch(const orc_problem *P, int64_t W, double *a, double *M, double
         chi2[i] = orc_chi2(n_tau, M + (size_t)i * n_tau, P->F, P->sigma);
     }
     return n_rec;
+}
+
+/* ---------------------------------------------------------------------------------------
+ * O8b  branching with a prescribed branching fraction:
+ *   "Parameter Delta is found numerically such that a given fraction of walkers is assigned a zero
+ *    multiplier."  Reading B6: Delta = 1/T is the smallest value on a doubling-then-bisection path for
+ *   which the comb multipliers of O8 (same Philox offset for every trial value) give at least
+ *   n0 = floor(fraction W + 1/2) zeros:
+ *     beta_0 = 1/(chi2_max - chi2_min); bracket by doubling / halving from beta_0 (at most 200 steps)
+ *     until Z(lo) < n0 <= Z(hi); 40 bisection steps on beta; T = 1/hi.
+ *   orc_branch_zeros counts the zero multipliers for a given T without touching the state.
+ *   Returns 0 and leaves *T_out = 0 when the population is degenerate (all chi2 equal) or n0 = 0.
+ * ------------------------------------------------------------------------------------- */
+int64_t orc_branch_zeros(const orc_problem *P, int64_t W, const double *chi2, double T, int64_t sweep)
+{
+    double cmin = chi2[0];
+    for (int64_t i = 1; i < W; ++i) if (chi2[i] < cmin) cmin = chi2[i];
+    uint64_t *C = (uint64_t *)malloc(sizeof(uint64_t) * (size_t)W);
+    uint64_t run = 0;
+    for (int64_t i = 0; i < W; ++i) {
+        run += (uint64_t)floor(exp(-(chi2[i] - cmin) / T) * 1099511627776.0);
+        C[i] = run;
+    }
+    const uint64_t S = run;
+    uint32_t ctr[4] = { 0u, (uint32_t)sweep, 0u, 1u };
+    uint32_t key[2] = { P->seed_lo, P->seed_hi };
+    uint32_t x[4];
+    orc_philox4x32_10(ctr, key, x);
+    const unsigned __int128 Xi = ((unsigned __int128)x[0] * S) >> 32;
+    uint64_t prev = 0;
+    int64_t zeros = 0;
+    for (int64_t i = 0; i < W; ++i) {
+        uint64_t cur = (uint64_t)(((unsigned __int128)C[i] * (uint64_t)W + Xi) / S);
+        if (cur == prev) zeros++;
+        prev = cur;
+    }
+    free(C);
+    return zeros;
+}
+
+int orc_branch_fraction_T(const orc_problem *P, int64_t W, const double *chi2, double fraction, int64_t sweep,
+                          double *T_out)
+{
+    *T_out = 0.0;
+    const int64_t n0 = (int64_t)floor(fraction * (double)W + 0.5);
+    double cmin = chi2[0], cmax = chi2[0];
+    for (int64_t i = 1; i < W; ++i) { if (chi2[i] < cmin) cmin = chi2[i]; if (chi2[i] > cmax) cmax = chi2[i]; }
+    if (n0 <= 0 || !(cmax > cmin)) return 0;
+    double lo, hi = 1.0 / (cmax - cmin);
+    if (orc_branch_zeros(P, W, chi2, 1.0 / hi, sweep) >= n0) {
+        lo = 0.5 * hi;
+        for (int it = 0; it < 200 && orc_branch_zeros(P, W, chi2, 1.0 / lo, sweep) >= n0; ++it) { hi = lo; lo = 0.5 * lo; }
+    } else {
+        lo = hi; hi = 2.0 * hi;
+        int it = 0;
+        for (; it < 200 && orc_branch_zeros(P, W, chi2, 1.0 / hi, sweep) < n0; ++it) { lo = hi; hi = 2.0 * hi; }
+        if (it == 200) return 0;               /* the fraction cannot be reached (e.g. n0 >= W) */
+    }
+    for (int it = 0; it < 40; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (orc_branch_zeros(P, W, chi2, 1.0 / mid, sweep) >= n0) hi = mid; else lo = mid;
+    }
+    *T_out = 1.0 / hi;
+    return 1;
 }
 
 /* ---------------------------------------------------------------------------------------

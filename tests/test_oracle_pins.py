@@ -555,3 +555,24 @@ def test_selfcool_protocol_runs_blocks_of_sweeps_branching_and_smoothing(tiny):
     wm = tiny.omega + 0.5 * tiny.domega
     np.testing.assert_allclose(o.a.sum(axis=1), tiny.A, rtol=1e-11)
     np.testing.assert_allclose((o.a * wm).sum(axis=1), tiny.B, rtol=1e-11)
+
+
+# ---- f2 branching fraction -----------------------------------------------------------
+def test_branch_fraction_finds_the_temperature_that_kills_the_asked_fraction(tiny):
+    """:174 'Delta is found numerically such that a given fraction of walkers is assigned a zero multiplier'.
+    zeros(T) is 0 for T -> inf (all weights equal: every m = 1), grows as T falls, and the T found is the edge:
+    zeros(T) >= n0 but a relative 1e-9 above it there are fewer."""
+    o = _oracle_for(tiny); o.init_walkers(400)
+    o.anneal(np.full(3, 1e5))
+    assert o.branch_zeros(1e30) == 0
+    zs = [o.branch_zeros(T) for T in np.std(o.chi2) * np.array([100.0, 10.0, 3.0, 1.0, 0.3, 0.1])]
+    assert zs[0] <= zs[2] <= zs[4] and zs[-1] > zs[0]
+    for frac in (0.25, 0.1, 0.5):
+        n0 = int(np.floor(frac * o.W + 0.5))
+        o2 = _oracle_for(tiny); o2.init_walkers(400, o.a.copy()); o2.chi2[:] = o.chi2; o2.sweep = o.sweep
+        T, n_rec, mult, donor = o2.branch_fraction(frac, 0.1)
+        assert T > 0 and mult.sum() == o.W and n_rec == (mult == 0).sum()
+        assert n_rec >= n0 and n_rec - n0 <= 0.02 * o.W                      # the comb moves in small integer jumps
+        assert o.branch_zeros(T) == n_rec and o.branch_zeros(T * (1 + 1e-9)) < n0
+    flat = _oracle_for(tiny); flat.init_walkers(16)                           # identical walkers: nothing to branch
+    assert flat.branch_fraction(0.25, 0.1)[0] == 0.0
