@@ -152,6 +152,18 @@ typedef struct {
 SAIL_API int sail_branch(sail_t *h, double T, double t_imprint, sail_branch_info *info, int32_t *mult_out,
                 int64_t *donor_out);
 
+/*
+ * sail_branch_fraction — the paper's own way of fixing the branching strength (:174, :220): "Delta is found
+ * numerically such that a given fraction of walkers is assigned a zero multiplier" (the paper branches a quarter of
+ * the walkers).  The inverse temperature Delta = 1/T of sail_branch is searched (bracketing from 1/(chi2_max -
+ * chi2_min), then 40 bisection steps; every trial runs the multiplier chain on the device with the same comb
+ * offset, reading B6) for the smallest value that gives at least floor(fraction W + 1/2) zeros; then the
+ * event runs at that temperature.  *T_found (HOST, may be NULL) receives it; 0 means no event happened (all residues
+ * equal, or fraction W rounds to 0).  Other arguments as sail_branch.  Synchronises the stream (once per trial).
+ */
+SAIL_API int sail_branch_fraction(sail_t *h, double fraction, double t_imprint, double *T_found, sail_branch_info *info,
+                                  int32_t *mult_out, int64_t *donor_out);
+
 /* sail_resync — recompute M = a K (dense W x N_omega x N_tau contraction) and chi^2 for all walkers. */
 SAIL_API int sail_resync(sail_t *h);
 
@@ -181,6 +193,8 @@ typedef struct {
     double  smooth_s;           /* smoothing amplitude applied before the branching; 0 = no smoothing (:190)        */
     int32_t branch;             /* 0: no branching                                                                  */
     int32_t reserved;
+    double  branch_fraction;    /* > 0: branch that fraction of the walkers (sail_branch_fraction; paper: 1/4, :220);
+                                 * 0: branch at the block's own 1/T (sail_branch)                                   */
     const double *T_override;   /* HOST [n_blocks] or NULL: use these temperatures instead of the rule (tests)      */
     sail_anneal_params anneal;  /* eta, Eq. 30 parameters, kernel form, traces for the sweeps of the blocks         */
 } sail_selfcool_params;

@@ -193,9 +193,10 @@ class Oracle:
         lib().orc_resync(C.byref(self.P), C.c_int64(self.W), _p(self.a), _p(self.M), _p(self.chi2))
 
     def anneal_selfcool(self, n_blocks, sweeps_per_block, n_boil, n_ramp, t_imprint=0.1, smooth_s=0.0,
-                        T_start=10.0, freeze_rate=1.0, T_override=None):
+                        T_start=10.0, freeze_rate=1.0, T_override=None, branch_fraction=0.0):
         """The paper's block protocol (:218-220) with self-cooling: per block, T from the population's residues, then
-        sweeps_per_block sweeps at that T, smoothing (if smooth_s > 0), one branching event at 1/T.  T_override[b]
+        sweeps_per_block sweeps at that T, smoothing (if smooth_s > 0), one branching event at 1/T (or, with
+        branch_fraction > 0, at the 1/T that gives that fraction of walkers multiplier zero: the paper's 1/4, :220).  T_override[b]
         replaces the rule (used by the parity tests to drive both sides with the same temperatures).
         Returns (T, chi2_ave, chi2_min) per block."""
         chi2_0 = float(np.mean(self.chi2))
@@ -209,7 +210,10 @@ class Oracle:
             self.anneal(np.full(sweeps_per_block, T))
             if smooth_s > 0.0:
                 self.smooth(smooth_s)
-            self.branch(T, t_imprint)
+            if branch_fraction > 0.0:
+                self.branch_fraction(branch_fraction, t_imprint)
+            else:
+                self.branch(T, t_imprint)
         return np.array(Ts), np.array(aves), np.array(mins)
 
     def smooth(self, s):

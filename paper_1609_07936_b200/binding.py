@@ -18,7 +18,7 @@ SAIL_OK, SAIL_ERR_ARG, SAIL_ERR_GRID, SAIL_ERR_ALLOC, SAIL_ERR_CUDA, SAIL_ERR_ST
 
 EXPORTS = ["sail_workspace_bytes", "sail_create", "sail_init_walkers", "sail_anneal", "sail_branch",
            "sail_resync", "sail_get", "sail_get_model", "sail_stats", "sail_set_walkers", "sail_set_sweep",
-           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak", "sail_microbench", "sail_smooth", "sail_chi2_stats", "sail_anneal_selfcool"]
+           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak", "sail_microbench", "sail_smooth", "sail_chi2_stats", "sail_anneal_selfcool", "sail_branch_fraction"]
 
 
 class SailError(RuntimeError):
@@ -43,7 +43,7 @@ class sail_selfcool_params(C.Structure):
     _fields_ = [("sweeps_per_block", C.c_int32), ("n_boil", C.c_int32), ("n_ramp", C.c_int32),
                 ("T_start", C.c_double), ("freeze_rate", C.c_double), ("t_imprint", C.c_double),
                 ("smooth_s", C.c_double), ("branch", C.c_int32), ("reserved", C.c_int32),
-                ("T_override", C.c_void_p), ("anneal", sail_anneal_params)]
+                ("branch_fraction", C.c_double), ("T_override", C.c_void_p), ("anneal", sail_anneal_params)]
 
 
 class sail_branch_info(C.Structure):
@@ -75,6 +75,8 @@ def lib():
         L.sail_branch.argtypes = [C.c_void_p, C.c_double, C.c_double, C.POINTER(sail_branch_info), C.c_void_p, C.c_void_p]
         L.sail_resync.argtypes = [C.c_void_p]
         L.sail_smooth.argtypes = [C.c_void_p, C.c_double]
+        L.sail_branch_fraction.argtypes = [C.c_void_p, C.c_double, C.c_double, C.POINTER(C.c_double),
+                                           C.POINTER(sail_branch_info), C.c_void_p, C.c_void_p]
         L.sail_chi2_stats.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         L.sail_anneal_selfcool.argtypes = [C.c_void_p, C.POINTER(sail_selfcool_params), C.c_int64, C.c_void_p,
                                            C.c_void_p, C.c_void_p]
@@ -205,13 +207,14 @@ class Sail:
         return mn.value, mean.value
 
     def anneal_selfcool(self, n_blocks, sweeps_per_block, n_boil, n_ramp, eta, t_imprint=0.1, smooth_s=0.0, T_start=10.0,
-                        freeze_rate=1.0, branch=True, T_override=None, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6,
+                        freeze_rate=1.0, branch=True, branch_fraction=0.0, T_override=None, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6,
                         lanes_per_walker=0):
         """The paper's block protocol with self-cooling (include/sail.h: sail_anneal_selfcool).
         Returns (T, chi2_ave, chi2_min), one entry per block."""
         p = sail_selfcool_params()
         p.sweeps_per_block, p.n_boil, p.n_ramp = sweeps_per_block, n_boil, n_ramp
         p.T_start, p.freeze_rate, p.t_imprint, p.smooth_s, p.branch = T_start, freeze_rate, t_imprint, smooth_s, int(branch)
+        p.branch_fraction = branch_fraction
         ov = _f64(T_override) if T_override is not None else None
         p.T_override = ov.ctypes.data if ov is not None else None
         p.anneal.eta, p.anneal.amp_mode, p.anneal.lanes_per_walker = eta, amp_mode, lanes_per_walker
@@ -226,6 +229,16 @@ class Sail:
         donor = np.empty(self.W, dtype=np.int64) if want_maps else None
         self._check(self._L.sail_branch(self._h, T, t_imprint, C.byref(info), _ptr(mult), _ptr(donor)))
         return info, mult, donor
+
+    def branch_fraction(self, fraction, t_imprint, want_maps=False):
+        """f2: branch so that `fraction` of the walkers get multiplier zero.  Returns (T_found, info, mult, donor)."""
+        info = sail_branch_info()
+        T = C.c_double(0.0)
+        mult = np.empty(self.W, dtype=np.int32) if want_maps else None
+        donor = np.empty(self.W, dtype=np.int64) if want_maps else None
+        self._check(self._L.sail_branch_fraction(self._h, C.c_double(fraction), C.c_double(t_imprint), C.byref(T),
+                                                 C.byref(info), _ptr(mult), _ptr(donor)))
+        return T.value, info, mult, donor
 
     def branch_async(self, T, t_imprint):
         self._check(self._L.sail_branch(self._h, T, t_imprint, None, None, None))

@@ -2,6 +2,8 @@
 // DESIGN.md §2): fixed-point weights -> integer prefix sum -> comb multipliers (sum m = W exactly) ->
 // donor map by binary search -> coalesced 128-bit imprint copy of (spectrum, model) + residue.
 #include "sail_internal.cuh"
+#include <math.h>
+#include <string.h>
 
 namespace sail {
 
@@ -322,7 +324,9 @@ __global__ void __launch_bounds__(128) imprint_tma_kernel(int n_omega, int n_tau
     if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
-int launch_branch(sail_handle *h, double T, double t_imprint)
+// weights -> scan -> multipliers -> scans -> donor map for inverse temperature 1/T; the number of recipients (zero
+// multipliers) ends up in scalars[2].  No walker state is touched.
+static int branch_plan(sail_handle *h, double T)
 {
     const long long W = h->W;
     BranchScratch &b = h->br;
@@ -342,6 +346,13 @@ int launch_branch(sail_handle *h, double T, double t_imprint)
     if (rc) return rc;
     donor_map_kernel<<<blocks, 256, 0, h->stream>>>(W, b.mult, b.scanA, b.scanB, b.donor_of, b.rec_list, b.scalars);
     SAIL_LAUNCH_OK(h, "donor_map_kernel");
+    return SAIL_OK;
+}
+
+static int branch_imprint(sail_handle *h, double t_imprint)
+{
+    const long long W = h->W;
+    BranchScratch &b = h->br;
     const int iblocks = (int)(W < (long long)h->num_sms * 8 ? W : (long long)h->num_sms * 8);
     // t = 1 with rows that are multiples of 16 bytes goes through the bulk-copy engine (measured on Stress, 187799
     // recipients: 1.05 ms against 1.31 ms with plain loads); for t < 1 the plain-load kernel is the faster one
@@ -373,6 +384,79 @@ int launch_branch(sail_handle *h, double T, double t_imprint)
                                                               h->st.a, h->st.mt, h->st.chi2, h->tab.Wj, h->tab.fj);
     SAIL_LAUNCH_OK(h, "imprint_kernel");
     return SAIL_OK;
+}
+
+int launch_branch(sail_handle *h, double T, double t_imprint)
+{
+    int rc = branch_plan(h, T);
+    if (rc) return rc;
+    return branch_imprint(h, t_imprint);
+}
+
+__global__ void chi2_max_kernel(long long W, const double *__restrict__ chi2, unsigned long long *dst)
+{
+    unsigned long long m = 0ull;                       // chi^2 >= 0: the bit patterns order like the values
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
+        const unsigned long long b = (unsigned long long)__double_as_longlong(chi2[i]);
+        m = b > m ? b : m;
+    }
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) {
+        const unsigned long long o = __shfl_xor_sync(0xffffffffu, m, off);
+        m = o > m ? o : m;
+    }
+    if ((threadIdx.x & 31) == 0) atomicMax(dst, m);
+}
+
+// SURVEY §8f row f2 (reading B6): 1/T such that `fraction` of the walkers get multiplier zero, found
+// by bracketing (doubling / halving from 1/(chi2_max - chi2_min)) and 40 bisection steps on 1/T; every trial runs the
+// multiplier chain on the device (same comb offset) and reads back one count.  Then the event itself at that T.
+int launch_branch_fraction(sail_handle *h, double fraction, double t_imprint, double *T_found)
+{
+    const long long W = h->W;
+    BranchScratch &b = h->br;
+    *T_found = 0.0;
+    const long long n0 = (long long)floor(fraction * (double)W + 0.5);
+    const int blocks = (int)((W + 255) / 256 < 1184 ? (W + 255) / 256 : 1184);
+    SAIL_CUDA_OK(h, cudaMemsetAsync(b.scalars, 0, 8 * sizeof(unsigned long long), h->stream));
+    SAIL_CUDA_OK(h, cudaMemsetAsync(b.scalars, 0xFF, sizeof(unsigned long long), h->stream));
+    chi2_min_kernel<<<blocks, 256, 0, h->stream>>>(W, h->st.chi2, b.scalars);
+    SAIL_LAUNCH_OK(h, "chi2_min_kernel");
+    chi2_max_kernel<<<blocks, 256, 0, h->stream>>>(W, h->st.chi2, b.scalars + 6);
+    SAIL_LAUNCH_OK(h, "chi2_max_kernel");
+    unsigned long long sc[8];
+    SAIL_CUDA_OK(h, cudaMemcpyAsync(sc, b.scalars, sizeof sc, cudaMemcpyDeviceToHost, h->stream));
+    SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
+    double cmin, cmax;
+    memcpy(&cmin, &sc[0], 8); memcpy(&cmax, &sc[6], 8);
+    if (n0 <= 0 || !(cmax > cmin)) return SAIL_OK;     // nothing to branch
+    int rc = SAIL_OK;
+    auto zeros = [&](double beta) -> long long {
+        if (rc) return 0;
+        rc = branch_plan(h, 1.0 / beta);
+        if (rc) return 0;
+        unsigned long long z = 0;
+        if (cudaMemcpyAsync(&z, b.scalars + 2, 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
+            cudaStreamSynchronize(h->stream) != cudaSuccess) { rc = set_err(h, SAIL_ERR_CUDA, "read-back of the recipient count failed"); return 0; }
+        return (long long)z;
+    };
+    double lo, hi = 1.0 / (cmax - cmin);
+    if (zeros(hi) >= n0) {
+        lo = 0.5 * hi;
+        for (int it = 0; it < 200 && zeros(lo) >= n0; ++it) { hi = lo; lo = 0.5 * lo; }
+    } else {
+        lo = hi; hi = 2.0 * hi;
+        int it = 0;
+        for (; it < 200 && zeros(hi) < n0; ++it) { lo = hi; hi = 2.0 * hi; }
+        if (it == 200) return rc;                      // the fraction cannot be reached
+    }
+    for (int it = 0; it < 40; ++it) {
+        const double mid = 0.5 * (lo + hi);
+        if (zeros(mid) >= n0) hi = mid; else lo = mid;
+    }
+    if (rc) return rc;
+    *T_found = 1.0 / hi;
+    return launch_branch(h, *T_found, t_imprint);
 }
 
 } // namespace sail

@@ -296,14 +296,8 @@ int sail_anneal(sail_t *h, const double *T_schedule, int64_t n_sweeps, const sai
     return SAIL_OK;
 }
 
-int sail_branch(sail_t *h, double T, double t_imprint, sail_branch_info *info, int32_t *mult_out, int64_t *donor_out)
+static int branch_outputs(sail_t *h, sail_branch_info *info, int32_t *mult_out, int64_t *donor_out)
 {
-    if (!h) return SAIL_ERR_ARG;
-    if (!h->initialised) return set_err(h, SAIL_ERR_STATE, "sail_branch before sail_init_walkers");
-    if (!(T > 0.0) || !(t_imprint >= 0.0 && t_imprint <= 1.0)) return set_err(h, SAIL_ERR_ARG, "need T > 0 and 0 <= t <= 1");
-    SAIL_CUDA_OK(h, cudaSetDevice(h->device));
-    int rc = launch_branch(h, T, t_imprint);
-    if (rc) return rc;
     if (info || mult_out || donor_out) {
         unsigned long long sc[8];
         SAIL_CUDA_OK(h, cudaMemcpyAsync(sc, h->br.scalars, sizeof sc, cudaMemcpyDeviceToHost, h->stream));
@@ -320,6 +314,38 @@ int sail_branch(sail_t *h, double T, double t_imprint, sail_branch_info *info, i
         }
     }
     return SAIL_OK;
+}
+
+int sail_branch(sail_t *h, double T, double t_imprint, sail_branch_info *info, int32_t *mult_out, int64_t *donor_out)
+{
+    if (!h) return SAIL_ERR_ARG;
+    if (!h->initialised) return set_err(h, SAIL_ERR_STATE, "sail_branch before sail_init_walkers");
+    if (!(T > 0.0) || !(t_imprint >= 0.0 && t_imprint <= 1.0)) return set_err(h, SAIL_ERR_ARG, "need T > 0 and 0 <= t <= 1");
+    SAIL_CUDA_OK(h, cudaSetDevice(h->device));
+    int rc = launch_branch(h, T, t_imprint);
+    if (rc) return rc;
+    return branch_outputs(h, info, mult_out, donor_out);
+}
+
+int sail_branch_fraction(sail_t *h, double fraction, double t_imprint, double *T_found, sail_branch_info *info,
+                         int32_t *mult_out, int64_t *donor_out)
+{
+    if (!h) return SAIL_ERR_ARG;
+    if (!h->initialised) return set_err(h, SAIL_ERR_STATE, "sail_branch_fraction before sail_init_walkers");
+    if (!(fraction >= 0.0 && fraction < 1.0) || !(t_imprint >= 0.0 && t_imprint <= 1.0))
+        return set_err(h, SAIL_ERR_ARG, "need 0 <= fraction < 1 and 0 <= t <= 1");
+    SAIL_CUDA_OK(h, cudaSetDevice(h->device));
+    double T = 0.0;
+    int rc = launch_branch_fraction(h, fraction, t_imprint, &T);
+    if (rc) return rc;
+    if (T_found) *T_found = T;
+    if (T == 0.0) {                                     // no event: degenerate population or nothing asked for
+        if (info) { info->n_recipients = 0; info->max_multiplier = 1; info->reserved = 0; info->chi2_min = 0.0; }
+        if (mult_out) for (int64_t i = 0; i < h->W; ++i) mult_out[i] = 1;
+        if (donor_out) for (int64_t i = 0; i < h->W; ++i) donor_out[i] = -1;
+        return SAIL_OK;
+    }
+    return branch_outputs(h, info, mult_out, donor_out);
 }
 
 int sail_resync(sail_t *h)

@@ -136,6 +136,7 @@ int launch_forward(sail_handle *h, int64_t w0, int64_t n);            // mt, chi
 int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sail_anneal_params *p,
                   int64_t sweeps_in_call, int64_t call_offset);
 int launch_branch(sail_handle *h, double T, double t_imprint);
+int launch_branch_fraction(sail_handle *h, double fraction, double t_imprint, double *T_found);   // row f2
 int launch_smooth(sail_handle *h, double s);                          // Eq. 27-29 + renormalisation + forward
 int launch_scale_model(sail_handle *h, double *dst);                  // dst[w][j] = c_j mt[w][j]
 int ensure_sweep_tables(sail_handle *h, int G);

@@ -93,7 +93,7 @@ int sail_anneal_selfcool(sail_t *h, const sail_selfcool_params *p, int64_t n_blo
     if (!h || !p) return SAIL_ERR_ARG;
     if (!h->initialised) return set_err(h, SAIL_ERR_STATE, "sail_anneal_selfcool before sail_init_walkers");
     if (n_blocks < 0 || p->sweeps_per_block < 1 || p->n_boil < 0 || p->n_ramp < 1 || !(p->T_start > 0.0) || !(p->freeze_rate > 0.0) ||
-        !(p->t_imprint >= 0.0 && p->t_imprint <= 1.0) || !(p->smooth_s >= 0.0 && p->smooth_s <= 0.5))
+        !(p->t_imprint >= 0.0 && p->t_imprint <= 1.0) || !(p->smooth_s >= 0.0 && p->smooth_s <= 0.5) || !(p->branch_fraction >= 0.0 && p->branch_fraction < 1.0))
         return set_err(h, SAIL_ERR_ARG, "bad self-cooling parameters");
     SAIL_CUDA_OK(h, cudaSetDevice(h->device));
     double chi2_0 = 0.0;
@@ -111,7 +111,11 @@ int sail_anneal_selfcool(sail_t *h, const sail_selfcool_params *p, int64_t n_blo
         for (auto &x : T) x = Tb;
         if ((rc = sail_anneal(h, T.data(), p->sweeps_per_block, &p->anneal))) return rc;
         if (p->smooth_s > 0.0 && (rc = sail_smooth(h, p->smooth_s))) return rc;
-        if (p->branch && (rc = sail_branch(h, Tb, p->t_imprint, nullptr, nullptr, nullptr))) return rc;
+        if (p->branch) {
+            if (p->branch_fraction > 0.0) rc = sail_branch_fraction(h, p->branch_fraction, p->t_imprint, nullptr, nullptr, nullptr, nullptr);
+            else rc = sail_branch(h, Tb, p->t_imprint, nullptr, nullptr, nullptr);
+            if (rc) return rc;
+        }
     }
     return SAIL_OK;
 }

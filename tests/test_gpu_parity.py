@@ -538,4 +538,49 @@ def test_selfcool_protocol_parity():
     o2 = _oracle(w, W)
     T2, _, _ = o2.anneal_selfcool(nb, k, n_boil, n_ramp, t_imprint=0.1, smooth_s=0.01)
     np.testing.assert_allclose(T2[:3], T[:3], rtol=1e-8)
+    # the paper's defaults for the branching step: a quarter of the walkers, t = 0.1 (:220)
+    s.init_walkers(W, w.A, w.B, SEED)
+    T3, _, _ = s.anneal_selfcool(4, k, n_boil, n_ramp, w.eta, t_imprint=0.1, branch_fraction=0.25)
+    o3 = _oracle(w, W)
+    o3.anneal_selfcool(4, k, n_boil, n_ramp, t_imprint=0.1, branch_fraction=0.25, T_override=T3)
+    a3, c3 = s.get()
+    np.testing.assert_allclose(a3, o3.a, rtol=0, atol=1e-9 * o3.a.max())
+    np.testing.assert_allclose(c3, o3.chi2, rtol=1e-7)
+    s.close()
+
+
+@pytest.mark.parametrize("W,frac,t", [(400, 0.25, 0.1), (3000, 0.25, 0.1), (3000, 0.1, 1.0), (64, 0.5, 0.3)])
+def test_branch_fraction_parity(W, frac, t):
+    """f2 (:174, :220; reading B6): from the same (a, chi^2) both sides find the same temperature (the bracketing /
+    bisection path is pure fp64 arithmetic steered by integer zero counts), the same multipliers and donor map, and
+    leave the same imprinted state; the asked fraction of walkers has multiplier zero."""
+    w = wl.make("tiny", simpson_intervals=20_000)
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED)
+    s.anneal(np.full(3, 1e5), w.eta)
+    a0, c0 = s.get()
+    o = _oracle(w, W, spectra=a0)
+    o.chi2[:] = c0
+    o.sweep = 3
+    Tg, info, mult, donor = s.branch_fraction(frac, t, want_maps=True)
+    To, n_rec, mo, do = o.branch_fraction(frac, t)
+    assert Tg == To and Tg > 0
+    assert (mult == mo).all() and (donor == do).all() and info.n_recipients == n_rec
+    n0 = int(np.floor(frac * W + 0.5))
+    assert mult.sum() == W and n0 <= n_rec <= n0 + 0.02 * W + 1
+    a1, c1 = s.get()
+    np.testing.assert_array_equal(a1, o.a)
+    rec = donor >= 0
+    np.testing.assert_allclose(c1[rec], o.chi2[rec], rtol=1e-8)
+    s.close()
+
+
+def test_branch_fraction_degenerate_population_is_a_no_op():
+    w = wl.make("tiny", simpson_intervals=20_000)
+    s = _sail(w, 32)
+    s.init_walkers(32, w.A, w.B, SEED)                       # identical walkers: all residues equal
+    a0, _ = s.get()
+    T, info, mult, donor = s.branch_fraction(0.25, 0.1, want_maps=True)
+    assert T == 0.0 and info.n_recipients == 0 and (mult == 1).all() and (donor == -1).all()
+    np.testing.assert_array_equal(s.get()[0], a0)
     s.close()
