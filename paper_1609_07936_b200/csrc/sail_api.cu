@@ -27,12 +27,13 @@ int set_err(sail_handle *h, int code, const char *fmt, ...)
 
 // ---- workspace layout ------------------------------------------------------------------------------
 struct Layout {
-    size_t off_omega, off_tau, off_c, off_Wj, off_fj, off_F, off_sigma, off_E, off_ET, off_ratio, off_invd, off_E0;
+    size_t off_omega, off_tau, off_c, off_Wj, off_fj, off_F, off_sigma, off_E, off_ET, off_ratio, off_invd, off_E0, off_T;
     size_t off_a, off_mt, off_chi2, off_y, off_nacc, off_neval;
     size_t off_ehat, off_scanA, off_scanB, off_bsums, off_mult, off_donor, off_reclist, off_scalars;
     size_t total;
 };
 constexpr size_t kE0Doubles = 16384;
+constexpr size_t kScheduleDoubles = 32768;   // temperature schedule slice (longer schedules are uploaded in pieces)
 
 static Layout make_layout(int n_omega, int n_tau, int64_t Wmax)
 {
@@ -46,6 +47,7 @@ static Layout make_layout(int n_omega, int n_tau, int64_t Wmax)
     L.off_sigma = take(n_tau * d);    L.off_E = take((size_t)n_omega * n_tau * d);
     L.off_ET = take((size_t)n_omega * n_tau * d);
     L.off_ratio = take(n_omega * d);  L.off_invd = take(n_omega * d);  L.off_E0 = take(kE0Doubles * d);
+    L.off_T = take(kScheduleDoubles * d);
     L.off_a = take(W * n_omega * d);  L.off_mt = take(W * n_tau * d);
     L.off_chi2 = take(W * d);         L.off_y = take(W * d);
     L.off_nacc = take(W * u);         L.off_neval = take(W * u);
@@ -174,9 +176,9 @@ int sail_create(sail_t **out, const double *omega, int32_t n_omega, const double
     auto fail = [&](int rc) { g_create_err = h->err; if (h->owns_workspace && h->workspace) cudaFree(h->workspace); delete h; return rc; };
     h->device = cfg->device;
     if (cudaSetDevice(h->device) != cudaSuccess) return fail(set_err(h, SAIL_ERR_CUDA, "cudaSetDevice(%d) failed", h->device));
-    cudaDeviceProp prop;
-    if (cudaGetDeviceProperties(&prop, h->device) != cudaSuccess) return fail(set_err(h, SAIL_ERR_CUDA, "cudaGetDeviceProperties failed"));
-    h->num_sms = prop.multiProcessorCount;
+    // one attribute, not cudaGetDeviceProperties: the full property query costs 10-20 ms on this driver
+    if (cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, h->device) != cudaSuccess)
+        return fail(set_err(h, SAIL_ERR_CUDA, "cudaDeviceGetAttribute failed"));
     h->stream = (cudaStream_t)cfg->stream;
     h->n_omega = n_omega; h->n_tau = n_tau; h->max_walkers = cfg->max_walkers;
     h->omega0 = w0; h->domega = dw; h->tau0 = t0; h->dtau = dt;
@@ -197,6 +199,7 @@ int sail_create(sail_t **out, const double *omega, int32_t n_omega, const double
     h->tab.omega = D(L.off_omega); h->tab.tau = D(L.off_tau); h->tab.c = D(L.off_c); h->tab.Wj = D(L.off_Wj);
     h->tab.fj = D(L.off_fj); h->tab.E = D(L.off_E); h->tab.ET = D(L.off_ET);
     h->sw_ratio = D(L.off_ratio); h->sw_invd = D(L.off_invd); h->sw_E0 = D(L.off_E0);
+    h->d_T = D(L.off_T); h->d_T_cap = kScheduleDoubles;
     h->st.a = D(L.off_a); h->st.mt = D(L.off_mt); h->st.chi2 = D(L.off_chi2); h->st.y = D(L.off_y);
     h->st.n_acc = U(L.off_nacc); h->st.n_eval = U(L.off_neval);
     h->br.ehat = U(L.off_ehat); h->br.scanA = U(L.off_scanA); h->br.scanB = U(L.off_scanB);
@@ -269,22 +272,23 @@ int sail_anneal(sail_t *h, const double *T_schedule, int64_t n_sweeps, const sai
         if (!(T_schedule[i] > 0.0)) return set_err(h, SAIL_ERR_ARG, "T_schedule[%lld] must be > 0", (long long)i);
     if (n_sweeps == 0) return SAIL_OK;
     SAIL_CUDA_OK(h, cudaSetDevice(h->device));
-    if ((size_t)n_sweeps > h->d_T_cap) {
-        if (h->d_T) { SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream)); cudaFree(h->d_T); h->d_T = nullptr; }
-        size_t cap = (size_t)n_sweeps < 4096 ? 4096 : (size_t)n_sweeps;
-        SAIL_CUDA_OK(h, cudaMalloc(&h->d_T, cap * sizeof(double)));
-        h->d_T_cap = cap;
-    }
-    SAIL_CUDA_OK(h, cudaMemcpyAsync(h->d_T, T_schedule, n_sweeps * sizeof(double), cudaMemcpyHostToDevice, h->stream));
-    int64_t done = 0;
+    // the schedule lives in a fixed slice of the workspace (no allocation, no cudaFree at destroy: cudaFree costs up to
+    // hundreds of ms on a busy context); longer schedules go through it piece by piece, stream-ordered
+    int64_t done = 0, piece_lo = 0, piece_hi = 0;
     while (done < n_sweeps) {
-        int64_t chunk = n_sweeps - done;
+        if (done == piece_hi) {
+            piece_lo = done;
+            piece_hi = done + (int64_t)h->d_T_cap < n_sweeps ? done + (int64_t)h->d_T_cap : n_sweeps;
+            SAIL_CUDA_OK(h, cudaMemcpyAsync(h->d_T, T_schedule + piece_lo, (size_t)(piece_hi - piece_lo) * sizeof(double),
+                                            cudaMemcpyHostToDevice, h->stream));
+        }
+        int64_t chunk = piece_hi - done;
         if (p->resync_every > 0) {
             const int64_t to_boundary = p->resync_every - (h->sweep % p->resync_every);
             if (to_boundary < chunk) chunk = to_boundary;
         }
         if (chunk > (1 << 30)) chunk = 1 << 30;
-        int rc = launch_sweeps(h, h->d_T + done, chunk, p, n_sweeps, done);
+        int rc = launch_sweeps(h, h->d_T + (done - piece_lo), chunk, p, n_sweeps, done);
         if (rc) return rc;
         h->sweep += chunk;
         done += chunk;
@@ -438,7 +442,6 @@ int sail_destroy(sail_t *h)
     if (!h) return SAIL_OK;
     cudaSetDevice(h->device);
     cudaStreamSynchronize(h->stream);
-    if (h->d_T) cudaFree(h->d_T);
     if (h->owns_workspace && h->workspace) cudaFree(h->workspace);
     delete h;
     return SAIL_OK;

@@ -78,7 +78,7 @@ struct sail_handle {
     double *sw_ratio = nullptr;  // [n_omega] exp(-omega_k G dtau)
     double *sw_invd = nullptr;   // [n_omega] 1/(k domega)
     double *sw_E0 = nullptr;     // direct: [n_omega][G]; factored: H[n_hi][G] then L[n_lo][G]
-    double *d_T = nullptr;       // device copy of the schedule chunk (library-owned, grows)
+    double *d_T = nullptr;       // device copy of the schedule piece in flight (a fixed slice of the workspace)
     size_t d_T_cap = 0;
     double *h_pinned = nullptr;  // small pinned staging buffer
     size_t h_pinned_cap = 0;

@@ -584,3 +584,16 @@ def test_branch_fraction_degenerate_population_is_a_no_op():
     assert T == 0.0 and info.n_recipients == 0 and (mult == 1).all() and (donor == -1).all()
     np.testing.assert_array_equal(s.get()[0], a0)
     s.close()
+
+
+def test_schedule_longer_than_the_device_slice_is_uploaded_in_pieces():
+    """sail_anneal keeps 32768 temperatures on the device at a time: a 33000-sweep call must equal the same sweeps
+    issued as 32768 + 232 (absolute sweep counter, stream-ordered re-upload of the slice)."""
+    w = wl.make("tiny", simpson_intervals=20_000)
+    T = wl.geometric_schedule(1.0, 1e-3, 33000)
+    s1 = _sail(w, 4); s1.init_walkers(4, w.A, w.B, SEED); s1.anneal(T, w.eta)
+    s2 = _sail(w, 4); s2.init_walkers(4, w.A, w.B, SEED); s2.anneal(T[:32768], w.eta); s2.anneal(T[32768:], w.eta)
+    a1, c1 = s1.get(); a2, c2 = s2.get()
+    np.testing.assert_array_equal(a1, a2)
+    np.testing.assert_array_equal(c1, c2)
+    s1.close(); s2.close()
