@@ -192,7 +192,8 @@ typedef struct {
     double  t_imprint;          /* imprint strength of the branching after every block (paper: 0.1, :220)          */
     double  smooth_s;           /* smoothing amplitude applied before the branching; 0 = no smoothing (:190)        */
     int32_t branch;             /* 0: no branching                                                                  */
-    int32_t reserved;
+    int32_t adapt;              /* 1: imprint strength and branching fraction of a block are multiplied by the block's
+                                 * acceptance rate relative to the largest one seen so far (:184, reading B7)          */
     double  branch_fraction;    /* > 0: branch that fraction of the walkers (sail_branch_fraction; paper: 1/4, :220);
                                  * 0: branch at the block's own 1/T (sail_branch)                                   */
     const double *T_override;   /* HOST [n_blocks] or NULL: use these temperatures instead of the rule (tests)      */

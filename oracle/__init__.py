@@ -193,7 +193,7 @@ class Oracle:
         lib().orc_resync(C.byref(self.P), C.c_int64(self.W), _p(self.a), _p(self.M), _p(self.chi2))
 
     def anneal_selfcool(self, n_blocks, sweeps_per_block, n_boil, n_ramp, t_imprint=0.1, smooth_s=0.0,
-                        T_start=10.0, freeze_rate=1.0, T_override=None, branch_fraction=0.0):
+                        T_start=10.0, freeze_rate=1.0, T_override=None, branch_fraction=0.0, adapt=False):
         """The paper's block protocol (:218-220) with self-cooling: per block, T from the population's residues, then
         sweeps_per_block sweeps at that T, smoothing (if smooth_s > 0), one branching event at 1/T (or, with
         branch_fraction > 0, at the 1/T that gives that fraction of walkers multiplier zero: the paper's 1/4, :220).  T_override[b]
@@ -201,6 +201,7 @@ class Oracle:
         Returns (T, chi2_ave, chi2_min) per block."""
         chi2_0 = float(np.mean(self.chi2))
         Ts, aves, mins = [], [], []
+        acc_prev, acc_max = int(self.acc.sum()), 0.0
         for b in range(n_blocks):
             ave, mn = float(np.mean(self.chi2)), float(np.min(self.chi2))
             T = selfcool_temperature(b, chi2_0, ave, mn, n_boil, n_ramp, T_start, freeze_rate)
@@ -210,10 +211,17 @@ class Oracle:
             self.anneal(np.full(sweeps_per_block, T))
             if smooth_s > 0.0:
                 self.smooth(smooth_s)
+            scale = 1.0
+            if adapt:       # :184, reading B7: strength follows the block's acceptance rate relative to the largest seen
+                acc_now = int(self.acc.sum())
+                rate = (acc_now - acc_prev) / (float(self.W) * float(sweeps_per_block) * float(self.P.n_omega))
+                acc_prev = acc_now
+                acc_max = max(acc_max, rate)
+                scale = rate / acc_max if acc_max > 0.0 else 0.0
             if branch_fraction > 0.0:
-                self.branch_fraction(branch_fraction, t_imprint)
+                self.branch_fraction(branch_fraction * scale, t_imprint * scale)
             else:
-                self.branch(T, t_imprint)
+                self.branch(T, t_imprint * scale)
         return np.array(Ts), np.array(aves), np.array(mins)
 
     def smooth(self, s):

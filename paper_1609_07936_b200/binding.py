@@ -42,7 +42,7 @@ class sail_anneal_params(C.Structure):
 class sail_selfcool_params(C.Structure):
     _fields_ = [("sweeps_per_block", C.c_int32), ("n_boil", C.c_int32), ("n_ramp", C.c_int32),
                 ("T_start", C.c_double), ("freeze_rate", C.c_double), ("t_imprint", C.c_double),
-                ("smooth_s", C.c_double), ("branch", C.c_int32), ("reserved", C.c_int32),
+                ("smooth_s", C.c_double), ("branch", C.c_int32), ("adapt", C.c_int32),
                 ("branch_fraction", C.c_double), ("T_override", C.c_void_p), ("anneal", sail_anneal_params)]
 
 
@@ -207,7 +207,7 @@ class Sail:
         return mn.value, mean.value
 
     def anneal_selfcool(self, n_blocks, sweeps_per_block, n_boil, n_ramp, eta, t_imprint=0.1, smooth_s=0.0, T_start=10.0,
-                        freeze_rate=1.0, branch=True, branch_fraction=0.0, T_override=None, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6,
+                        freeze_rate=1.0, branch=True, branch_fraction=0.0, adapt=False, T_override=None, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6,
                         lanes_per_walker=0):
         """The paper's block protocol with self-cooling (include/sail.h: sail_anneal_selfcool).
         Returns (T, chi2_ave, chi2_min), one entry per block."""
@@ -215,6 +215,7 @@ class Sail:
         p.sweeps_per_block, p.n_boil, p.n_ramp = sweeps_per_block, n_boil, n_ramp
         p.T_start, p.freeze_rate, p.t_imprint, p.smooth_s, p.branch = T_start, freeze_rate, t_imprint, smooth_s, int(branch)
         p.branch_fraction = branch_fraction
+        p.adapt = int(adapt)
         ov = _f64(T_override) if T_override is not None else None
         p.T_override = ov.ctypes.data if ov is not None else None
         p.anneal.eta, p.anneal.amp_mode, p.anneal.lanes_per_walker = eta, amp_mode, lanes_per_walker

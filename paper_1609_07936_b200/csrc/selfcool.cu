@@ -65,6 +65,28 @@ int launch_chi2_stats(sail_handle *h, double *host_min, double *host_mean)
     return SAIL_OK;
 }
 
+// exact (integer) total of the accepted-move counters: the acceptance rate of a block is a difference of two of these
+__global__ void sum_u64_kernel(long long W, const unsigned long long *__restrict__ v, unsigned long long *dst)
+{
+    unsigned long long s = 0ull;
+    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) s += v[i];
+#pragma unroll
+    for (int off = 16; off > 0; off >>= 1) s += __shfl_xor_sync(0xffffffffu, s, off);
+    if ((threadIdx.x & 31) == 0) atomicAdd(dst, s);
+}
+
+static int accepted_total(sail_handle *h, unsigned long long *total)
+{
+    unsigned long long *dst = h->br.scalars + 7;
+    SAIL_CUDA_OK(h, cudaMemsetAsync(dst, 0, 8, h->stream));
+    const int blocks = (int)((h->W + 255) / 256 < 256 ? (h->W + 255) / 256 : 256);
+    sum_u64_kernel<<<blocks, 256, 0, h->stream>>>(h->W, h->st.n_acc, dst);
+    SAIL_LAUNCH_OK(h, "sum_u64_kernel");
+    SAIL_CUDA_OK(h, cudaMemcpyAsync(total, dst, 8, cudaMemcpyDeviceToHost, h->stream));
+    SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
+    return SAIL_OK;
+}
+
 // readings C1-C3: the temperature of block b from the residues measured before it
 static double selfcool_T(int64_t b, double chi2_0, double ave, double mn, const sail_selfcool_params *p)
 {
@@ -96,7 +118,9 @@ int sail_anneal_selfcool(sail_t *h, const sail_selfcool_params *p, int64_t n_blo
         !(p->t_imprint >= 0.0 && p->t_imprint <= 1.0) || !(p->smooth_s >= 0.0 && p->smooth_s <= 0.5) || !(p->branch_fraction >= 0.0 && p->branch_fraction < 1.0))
         return set_err(h, SAIL_ERR_ARG, "bad self-cooling parameters");
     SAIL_CUDA_OK(h, cudaSetDevice(h->device));
-    double chi2_0 = 0.0;
+    double chi2_0 = 0.0, acc_max = 0.0;
+    unsigned long long acc_prev = 0ull;
+    if (p->adapt) { int rc0 = accepted_total(h, &acc_prev); if (rc0) return rc0; }
     std::vector<double> T((size_t)p->sweeps_per_block);
     for (int64_t b = 0; b < n_blocks; ++b) {
         double mn = 0.0, ave = 0.0;
@@ -111,9 +135,19 @@ int sail_anneal_selfcool(sail_t *h, const sail_selfcool_params *p, int64_t n_blo
         for (auto &x : T) x = Tb;
         if ((rc = sail_anneal(h, T.data(), p->sweeps_per_block, &p->anneal))) return rc;
         if (p->smooth_s > 0.0 && (rc = sail_smooth(h, p->smooth_s))) return rc;
+        // :184 (reading B7): less imprinting and a smaller branching fraction as the acceptance rate falls
+        double scale = 1.0;
+        if (p->adapt) {
+            unsigned long long acc_now = 0ull;
+            if ((rc = accepted_total(h, &acc_now))) return rc;
+            const double rate = (double)(acc_now - acc_prev) / ((double)h->W * (double)p->sweeps_per_block * (double)h->n_omega);
+            acc_prev = acc_now;
+            if (rate > acc_max) acc_max = rate;
+            scale = acc_max > 0.0 ? rate / acc_max : 0.0;
+        }
         if (p->branch) {
-            if (p->branch_fraction > 0.0) rc = sail_branch_fraction(h, p->branch_fraction, p->t_imprint, nullptr, nullptr, nullptr, nullptr);
-            else rc = sail_branch(h, Tb, p->t_imprint, nullptr, nullptr, nullptr);
+            if (p->branch_fraction > 0.0) rc = sail_branch_fraction(h, p->branch_fraction * scale, p->t_imprint * scale, nullptr, nullptr, nullptr, nullptr);
+            else rc = sail_branch(h, Tb, p->t_imprint * scale, nullptr, nullptr, nullptr);
             if (rc) return rc;
         }
     }

@@ -540,9 +540,10 @@ def test_selfcool_protocol_parity():
     np.testing.assert_allclose(T2[:3], T[:3], rtol=1e-8)
     # the paper's defaults for the branching step: a quarter of the walkers, t = 0.1 (:220)
     s.init_walkers(W, w.A, w.B, SEED)
-    T3, _, _ = s.anneal_selfcool(4, k, n_boil, n_ramp, w.eta, t_imprint=0.1, branch_fraction=0.25)
+    # ... reduced with the acceptance rate (:184)
+    T3, _, _ = s.anneal_selfcool(5, k, n_boil, n_ramp, w.eta, t_imprint=0.1, branch_fraction=0.25, adapt=True)
     o3 = _oracle(w, W)
-    o3.anneal_selfcool(4, k, n_boil, n_ramp, t_imprint=0.1, branch_fraction=0.25, T_override=T3)
+    o3.anneal_selfcool(5, k, n_boil, n_ramp, t_imprint=0.1, branch_fraction=0.25, adapt=True, T_override=T3)
     a3, c3 = s.get()
     np.testing.assert_allclose(a3, o3.a, rtol=0, atol=1e-9 * o3.a.max())
     np.testing.assert_allclose(c3, o3.chi2, rtol=1e-7)
