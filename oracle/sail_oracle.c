@@ -170,6 +170,7 @@ typedef struct {
     double amp_p, amp_m;   /* Eq. 30 parameters (paper: p = 1, m = 2)          */
     double y_min;          /* floor of y (reading G7)                          */
     uint32_t seed_lo, seed_hi;
+    int32_t walk_len;      /* length L of the index-selection walk (section 2.3); 0 = uniform p, s (reading G11) */
 } orc_problem;
 
 /* One traced move (what the parity tests compare). */
@@ -209,7 +210,25 @@ int orc_move(const orc_problem *P, int64_t walker, int64_t sweep, int32_t move, 
 
     int32_t p = (int32_t)(((uint64_t)x[0] * (uint64_t)n_omega) >> 32);
     int32_t s = (int32_t)(((uint64_t)x[1] * (uint64_t)(n_omega - 1)) >> 32);
+    /* Section 2.3 (reading F4): "a truncated Markov walk in the space of the
+     * spectral coefficients" selects p and s; zero length = uniform, infinite length = P(j) = a_j / A.  The walk is
+     * Metropolis on the bin index with uniform candidates: j <- c if u a_j < a_c.  Step l = 0 .. L-1 draws
+     * Philox(ctr = (walker, sweep, move, 2 + l)) = (candidate for p, u for p, candidate for s, u for s); the whole
+     * p-walk runs first, then s starts from its uniform draw on the bins other than the final p and walks on those. */
+    for (int l = 0; l < P->walk_len; ++l) {
+        uint32_t cw[4] = { (uint32_t)walker, (uint32_t)sweep, (uint32_t)move, (uint32_t)(2 + l) }, xw[4];
+        orc_philox4x32_10(cw, key, xw);
+        int32_t c = (int32_t)(((uint64_t)xw[0] * (uint64_t)n_omega) >> 32);
+        if (orc_u01(xw[1]) * a[p] < a[c]) p = c;
+    }
     if (s >= p) s += 1;
+    for (int l = 0; l < P->walk_len; ++l) {
+        uint32_t cw[4] = { (uint32_t)walker, (uint32_t)sweep, (uint32_t)move, (uint32_t)(2 + l) }, xw[4];
+        orc_philox4x32_10(cw, key, xw);
+        int32_t c = (int32_t)(((uint64_t)xw[2] * (uint64_t)(n_omega - 1)) >> 32);
+        if (c >= p) c += 1;
+        if (orc_u01(xw[3]) * a[s] < a[c]) s = c;
+    }
     double u_rho = orc_u01(x[2]), u_acc = orc_u01(x[3]);
     double rho = 1.0 - y * P->eta * (2.0 * u_rho - 1.0);
 

@@ -576,3 +576,60 @@ def test_branch_fraction_finds_the_temperature_that_kills_the_asked_fraction(tin
         assert o.branch_zeros(T) == n_rec and o.branch_zeros(T * (1 + 1e-9)) < n0
     flat = _oracle_for(tiny); flat.init_walkers(16)                           # identical walkers: nothing to branch
     assert flat.branch_fraction(0.25, 0.1)[0] == 0.0
+
+
+# ---- f4 index selection by a truncated Markov walk -------------------------------------
+def _selected_indices(o, a, n_moves, sweep=0):
+    """p, s the oracle selects for moves 0..n_moves-1 of walker 0 on the FIXED spectrum a (T = 1e-300: nothing is
+    ever accepted, so a never changes)."""
+    ps = np.zeros((n_moves, 2), dtype=int)
+    for m in range(n_moves):
+        aa = a.copy(); M = np.zeros(o.P.n_tau); tr = o.move_raw(0, sweep, m, 1e-300, aa, M)
+        ps[m] = tr["p"], tr["s"]
+    return ps
+
+
+def test_index_walk_limits_uniform_and_proportional_to_a(tiny):
+    """:158 'If the walk has zero length, indices are selected randomly and uniformly ... In the limit of infinitely
+    long walks, the indices are selected according to probability P(j) = a_j / A.'"""
+    N = tiny.n_omega
+    a = np.full(N, 1e-3); a[5] = 3.0; a[20] = 1.0; a[40] = 2.0            # three heavy bins: P = 1/2, 1/6, 1/3
+    n = 3000
+    o0 = _oracle_for(tiny, walk_len=0); o0.init_walkers(1)
+    ps0 = _selected_indices(o0, a, n)
+    assert (ps0[:, 0] != ps0[:, 1]).all()
+    frac_heavy0 = np.isin(ps0[:, 0], [5, 20, 40]).mean()
+    assert abs(frac_heavy0 - 3.0 / N) < 0.02                                # uniform: heavy bins are not preferred
+    oL = _oracle_for(tiny, walk_len=1000); oL.init_walkers(1)     # ~47 proposals of a heavy bin per walk: mixed
+    psL = _selected_indices(oL, a, n)
+    assert (psL[:, 0] != psL[:, 1]).all()
+    w = a / a.sum()
+    for j in (5, 20, 40):
+        assert abs((psL[:, 0] == j).mean() - w[j]) < 4 * np.sqrt(w[j] * (1 - w[j]) / n) + 0.01
+    # s is drawn from the same law restricted to the bins other than p
+    sel = psL[:, 0] == 5
+    cond = a.copy(); cond[5] = 0.0; cond /= cond.sum()
+    for j in (20, 40):
+        assert abs((psL[sel, 1] == j).mean() - cond[j]) < 4 * np.sqrt(cond[j] * (1 - cond[j]) / sel.sum()) + 0.02
+
+
+def test_index_walk_one_step_is_the_metropolis_rule_on_a(tiny):
+    """One walk step by hand: from the uniform start j, the candidate c (Philox stream 2) replaces it iff u a_j < a_c."""
+    N = tiny.n_omega
+    rng = np.random.default_rng(7)
+    a = rng.random(N) + 0.05
+    o1 = _oracle_for(tiny, walk_len=1); o1.init_walkers(1)
+    o0 = _oracle_for(tiny, walk_len=0); o0.init_walkers(1)
+    ps1, ps0 = _selected_indices(o1, a, 200), _selected_indices(o0, a, 200)
+    key = (o1.P.seed_lo, o1.P.seed_hi)
+    moved = 0
+    for m in range(200):
+        x = oracle.philox4x32_10((0, 0, m, 2), key)
+        x0 = oracle.philox4x32_10((0, 0, m, 0), key)
+        p0 = (int(x0[0]) * N) >> 32
+        c = (int(x[0]) * N) >> 32
+        u = (int(x[1]) + 0.5) / 2.0 ** 32
+        p1 = c if u * a[p0] < a[c] else p0
+        assert ps0[m, 0] == p0 and ps1[m, 0] == p1
+        moved += p1 != p0
+    assert 20 < moved < 190
