@@ -121,6 +121,10 @@ typedef struct {
     int64_t trace_lo, trace_hi;  /* walkers whose moves are traced; lo == hi: none                 */
     sail_trace_rec *trace;   /* DEVICE [(hi-lo)][n_sweeps][n_omega] or NULL                        */
     uint8_t *flags;          /* DEVICE [W][n_sweeps][n_omega] per-move flag bytes, or NULL         */
+    int32_t walk_length;     /* section 2.3 (:156-158): p and s by a truncated Markov walk of this many steps on the
+                              * current spectrum (j <- uniform candidate c if u a_j < a_c); 0 = uniform p, s.  The
+                              * proposal then depends on the state, so the plain (unscreened) kernel runs it.   */
+    int32_t reserved;
 } sail_anneal_params;
 
 /*

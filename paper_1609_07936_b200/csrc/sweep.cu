@@ -57,7 +57,7 @@ __device__ __forceinline__ void propose(const SweepArgs &P, uint32_t walker, uin
 // ---- one walker per WARP, register-lean (<= 72 registers: 28 resident warps per SM = 7 per sub-partition) ------
 // No software pipeline (the other six warps of the sub-partition hide
 // the latencies), every decision is warp-uniform, so infeasible and rejected moves branch around the work.
-template <int C, int MAXW, bool FACT, bool TRACE>
+template <int C, int MAXW, bool FACT, bool TRACE, bool WALK>
 __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kernel_warp(const SweepArgs P)
 {
     constexpr int G = 32;
@@ -125,15 +125,49 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                 __syncwarp();
                 const uint32_t r_end = rbase + (uint32_t)(nb * kRecBytes);
                 for (uint32_t r = rbase; r != r_end; r += kRecBytes) {
-                    const int4 r0 = lds_s32x4(r);
-                    const double2 dd = lds_f64x2(r + 16);
+                    int4 r0 = lds_s32x4(r);
+                    double2 dd = lds_f64x2(r + 16);
                     const double alpha = __hiloint2double(r0.w, r0.z);
+                    double2 rr = lds_f64x2(r + 48);
+                    const double2 th = lds_f64x2(r + 32);
+                    if (WALK) {
+                        // ---- index selection by a truncated Markov walk (section 2.3; reading F4):
+                        // Metropolis on the bin index with uniform candidates, j <- c if u a_j < a_c, L steps for p,
+                        // then L steps for s on the bins other than p.  The walk reads the CURRENT spectrum (a ratio:
+                        // the lazy scale cancels), so it runs at the move's turn, redundantly in every lane, and the
+                        // index-dependent half of the proposal (Eq. 20-21, the recurrence ratios) is redone here in the
+                        // operation order of propose().
+                        const uint32_t mv = (uint32_t)(m0 + (int)((r - rbase) / kRecBytes));
+                        const uint32_t sw = (uint32_t)(P.sweep0 + isw);
+                        int p = r0.x, s = r0.y;
+                        const int sraw = s - (s > p ? 1 : 0);
+                        for (int l = 0; l < P.walk_len; ++l) {
+                            uint32_t xw[4];
+                            philox4x32_10((uint32_t)w, sw, mv, (uint32_t)(2 + l), P.seed_lo, P.seed_hi, xw);
+                            const int c = (int)__umulhi(xw[0], (uint32_t)n_omega);
+                            const double u = ((double)xw[1] + 0.5) * 2.3283064365386962890625e-10;
+                            if (__dmul_rn(u, ldg_f64(elem_ptr(a_all, wbase + (uint32_t)p))) < ldg_f64(elem_ptr(a_all, wbase + (uint32_t)c))) p = c;
+                        }
+                        s = sraw + (sraw >= p ? 1 : 0);
+                        for (int l = 0; l < P.walk_len; ++l) {
+                            uint32_t xw[4];
+                            philox4x32_10((uint32_t)w, sw, mv, (uint32_t)(2 + l), P.seed_lo, P.seed_hi, xw);
+                            int c = (int)__umulhi(xw[2], (uint32_t)(n_omega - 1));
+                            c += (c >= p) ? 1 : 0;
+                            const double u = ((double)xw[3] + 0.5) * 2.3283064365386962890625e-10;
+                            if (__dmul_rn(u, ldg_f64(elem_ptr(a_all, wbase + (uint32_t)s))) < ldg_f64(elem_ptr(a_all, wbase + (uint32_t)c))) s = c;
+                        }
+                        const double omr = -alpha;                       // 1 - rho, exact like alpha = rho - 1
+                        const int dps = p - s;
+                        const double inv = (dps > 0) ? s_invd[dps] : -s_invd[-dps];
+                        dd.x = __dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[s]))), inv);
+                        dd.y = -__dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[p]))), inv);
+                        rr = make_double2(s_ratio[p], s_ratio[s]);
+                        r0.x = p; r0.y = s;
+                    }
                     double *const pp = elem_ptr(a_all, wbase + (uint32_t)r0.x);
                     double *const ps = elem_ptr(a_all, wbase + (uint32_t)r0.y);
                     const double a_p = ldg_f64(pp), a_s = ldg_f64(ps);
-                    // issued before the feasibility branch so that their latency overlaps the positivity test
-                    const double2 rr = lds_f64x2(r + 48);
-                    const double2 th = lds_f64x2(r + 32);
                     double ep, es;
                     if (FACT) {
                         ep = lds_f64(e0_lane + (uint32_t)((r0.x >> fshift) * (G * 8))) * lds_f64(e0_lo + (uint32_t)((r0.x & fmask) * (G * 8)));
@@ -489,13 +523,14 @@ int ensure_sweep_tables(sail_handle *h, int G)
 }
 
 // ---- dispatch -----------------------------------------------------------------------------------------
-// MODE 1: lean one walker per warp (sweep_kernel_warp), 2: screened one walker per warp (sweep_kernel_mask),
+// MODE 1: lean one walker per warp (sweep_kernel_warp), 4: the same with the index walk of section 2.3,
+//      2: screened one walker per warp (sweep_kernel_mask),
 //      3: the same with 2 Wj in registers
 template <int C, int MAXW, bool FACT, bool TRACE, int MODE, int DMMA = 0>
 static int launch_variant(sail_handle *h, SweepArgs &args)
 {
     constexpr int G = 32;
-    constexpr int rec_bytes = (MODE >= 2) ? kRecMaskBytes : kRecBytes;
+    constexpr int rec_bytes = (MODE == 2 || MODE == 3) ? kRecMaskBytes : kRecBytes;
     args.n_groups = args.W;
     int warps = (int)((args.n_groups + h->num_sms - 1) / h->num_sms);
     if (warps > MAXW) warps = MAXW;
@@ -510,7 +545,8 @@ static int launch_variant(sail_handle *h, SweepArgs &args)
     void (*kern)(const SweepArgs);
     if constexpr (MODE == 3) kern = sweep_kernel_mask<C, MAXW, FACT, TRACE, true, DMMA>;
     else if constexpr (MODE == 2) kern = sweep_kernel_mask<C, MAXW, FACT, TRACE, false, DMMA>;
-    else kern = sweep_kernel_warp<C, MAXW, FACT, TRACE>;
+    else if constexpr (MODE == 4) kern = sweep_kernel_warp<C, MAXW, FACT, TRACE, true>;
+    else kern = sweep_kernel_warp<C, MAXW, FACT, TRACE, false>;
     SAIL_CUDA_OK(h, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     int resident = 0;
     SAIL_CUDA_OK(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&resident, kern, warps * 32, smem));
@@ -537,6 +573,9 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     const int req = p->lanes_per_walker;
     if (!(req == 0 || req == 8 || req == 16 || req == 32 || (req >= 34 && req <= 37)))
         return set_err(h, SAIL_ERR_ARG, "lanes_per_walker=%d is not one of 0, 8, 16, 32, 34..37", req);
+    if (p->walk_length < 0 || p->walk_length > 4096) return set_err(h, SAIL_ERR_ARG, "walk_length=%d outside [0, 4096]", p->walk_length);
+    if (p->walk_length > 0 && !(req == 0 || req == 32 || req == 34))
+        return set_err(h, SAIL_ERR_ARG, "walk_length > 0 runs on the plain one-walker-per-warp kernel: lanes_per_walker must be 0, 32 or 34");
     const int G = pick_lanes(req);
     // (16 lanes per walker win the first sweeps of Branching, 0.281 against 0.269, but lose over the whole anneal,
     // 0.270 against 0.280: auto stays with one walker per warp)
@@ -564,12 +603,13 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     a.a = h->st.a; a.mt = h->st.mt; a.chi2 = h->st.chi2; a.y = h->st.y;
     a.n_acc = h->st.n_acc; a.n_eval = h->st.n_eval;
     a.T = d_T; a.sweep0 = h->sweep; a.n_sweeps = (int)n_sweeps;
+    a.walk_len = p->walk_length;
     a.trace_lo = p->trace_lo; a.trace_hi = p->trace_hi; a.trace = p->trace; a.flags = p->flags;
     a.call_sweeps = sweeps_in_call; a.call_off = call_offset;
     const bool trace = (p->trace != nullptr) || (p->flags != nullptr);
 
     // grouped screened kernel (sweep_grp.cu): 8 / 16 lanes per walker, 36 = its one-walker-per-warp instance
-    if (req == 8 || req == 16 || req == 36) return launch_sweep_grp(h, a, G, C, trace, 0);
+    if (a.walk_len == 0 && (req == 8 || req == 16 || req == 36)) return launch_sweep_grp(h, a, G, C, trace, 0);
 
 #define SAIL_VARIANT(CC, MW, MODE)                                                                                  \
     {                                                                                                                   \
@@ -580,6 +620,11 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     {                                                                                                                   \
         if (a.fact) return trace ? launch_variant<CC, MW, true, true, MODE, 1>(h, a) : launch_variant<CC, MW, true, false, MODE, 1>(h, a);   \
         return trace ? launch_variant<CC, MW, false, true, MODE, 1>(h, a) : launch_variant<CC, MW, false, false, MODE, 1>(h, a);             \
+    }
+    if (a.walk_len > 0) {                              // index selection by a truncated walk: the plain form only
+        if (C <= 4) SAIL_VARIANT(4, 28, 4)
+        if (C <= 8) SAIL_VARIANT(8, 16, 4)
+        SAIL_VARIANT(16, 12, 4)
     }
     if (req == 0 || req == 32) {                       // screened, DMMA warp sum (default)
         if (C <= 4) SAIL_VARIANT_D(4, 28, 2)

@@ -18,6 +18,7 @@ struct SweepArgs {
     const double *T;
     long long sweep0;
     int n_sweeps;
+    int walk_len;                      // length of the index-selection walk (section 2.3); 0 = uniform indices
     long long trace_lo, trace_hi;
     sail_trace_rec *trace;
     uint8_t *flags;
