@@ -364,7 +364,31 @@ def extra_workloads(torch, Sail, dev_index, peaks):
         out[key] = {"seconds": t_br, "recipients": n_rec, "algorithmic_GB": algo_bytes / 1e9,
                     "achieved_GBps": algo_bytes / t_br / 1e9, "frac_of_measured_hbm": algo_bytes / t_br / 1e9 / hbm,
                     "note": "whole event (12 launches + info read-back); donors with several recipients are re-read from L2"}
+    # f2: the paper's branching step (a quarter of the walkers, t = 0.1): search of 1/T (one multiplier chain and one
+    # 8-byte read-back per trial) + the event itself; f1: the two-kernel residue statistics of the self-cooling schedule
+    s.init_walkers(w.W, w.A, w.B, w.rng_seed)
+    s.anneal(w.schedule[:1], **p)
+    l0 = s.launch_count()
+    box = {}
+    t_bf = timed(lambda: box.update(r=s.branch_fraction(0.25, 0.1)))
+    out["stress_branch_fraction_0.25"] = {"seconds": t_bf, "T_found": box["r"][0], "recipients": int(box["r"][1].n_recipients),
+                                          "kernel_launches": int(s.launch_count() - l0)}
+    out["stress_chi2_stats"] = {"seconds": timed(lambda: s.chi2_stats(), reps=5)}
     s.close()
+    # f4: sweeps with the index-selection walk (2 steps) on Small; it runs on the plain kernel (state-dependent proposals)
+    w2 = wl.make("small")
+    s2 = Sail(w2.omega, w2.tau, w2.F, w2.sigma, max_walkers=w2.W, device=dev_index)
+    s2.init_walkers(w2.W, w2.A, w2.B, w2.rng_seed)
+    p2 = anneal_params(w2)
+    s2.anneal(w2.schedule[:5], walk_length=2, **p2)
+    _, ev0, _ = s2.stats()
+    n2 = 100
+    t_w = timed(lambda: s2.anneal(w2.schedule[5:5 + n2], walk_length=2, **p2))
+    _, ev1, _ = s2.stats()
+    out["small_sweeps_walk2"] = {"attempted_moves_per_s": w2.W * n2 * w2.n_omega / t_w, "seconds": t_w,
+                                 "evaluated_fraction": float((ev1 - ev0).sum()) / (w2.W * n2 * w2.n_omega),
+                                 "roofline_frac": DFMA_PER_TAU_POINT * w2.n_tau * float((ev1 - ev0).sum()) / t_w / peak}
+    s2.close()
     return out
 
 

@@ -61,6 +61,7 @@ template <int C, int MAXW, bool FACT, bool TRACE, bool WALK>
 __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kernel_warp(const SweepArgs P)
 {
     constexpr int G = 32;
+    constexpr int kRecBytes = WALK ? 96 : sail::kRecBytes;   // WALK: + the Philox words of the first two walk steps
     extern __shared__ __align__(16) unsigned char smem[];
     double *s_ratio = reinterpret_cast<double *>(smem);
     const int n_omega = P.n_omega;
@@ -122,6 +123,19 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                 if (lane < nb)
                     propose(P, (uint32_t)w, (uint32_t)(P.sweep0 + isw), (uint32_t)(m0 + lane), P.y[w], P.T[isw],
                             s_ratio, s_invd, s_wm, my_rec_w);
+                if (WALK) {
+                    // the random words of the walk do not depend on the state: the first two steps are drawn here, one
+                    // move per lane, and staged behind the record
+                    if (lane < nb) {
+#pragma unroll
+                        for (int l = 0; l < 2; ++l) {
+                            uint32_t xw[4] = {0u, 0u, 0u, 0u};
+                            if (l < P.walk_len)
+                                philox4x32_10((uint32_t)w, (uint32_t)(P.sweep0 + isw), (uint32_t)(m0 + lane), (uint32_t)(2 + l), P.seed_lo, P.seed_hi, xw);
+                            *reinterpret_cast<uint4 *>(my_rec_w + 64 + 16 * l) = make_uint4(xw[0], xw[1], xw[2], xw[3]);
+                        }
+                    }
+                }
                 __syncwarp();
                 const uint32_t r_end = rbase + (uint32_t)(nb * kRecBytes);
                 for (uint32_t r = rbase; r != r_end; r += kRecBytes) {
@@ -141,9 +155,17 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                         const uint32_t sw = (uint32_t)(P.sweep0 + isw);
                         int p = r0.x, s = r0.y;
                         const int sraw = s - (s > p ? 1 : 0);
+                        auto walk_words = [&](int l, uint32_t (&xw)[4]) {
+                            if (l < 2) {
+                                const int4 q = lds_s32x4(r + 64 + 16 * l);
+                                xw[0] = (uint32_t)q.x; xw[1] = (uint32_t)q.y; xw[2] = (uint32_t)q.z; xw[3] = (uint32_t)q.w;
+                            } else {
+                                philox4x32_10((uint32_t)w, sw, mv, (uint32_t)(2 + l), P.seed_lo, P.seed_hi, xw);
+                            }
+                        };
                         for (int l = 0; l < P.walk_len; ++l) {
                             uint32_t xw[4];
-                            philox4x32_10((uint32_t)w, sw, mv, (uint32_t)(2 + l), P.seed_lo, P.seed_hi, xw);
+                            walk_words(l, xw);
                             const int c = (int)__umulhi(xw[0], (uint32_t)n_omega);
                             const double u = ((double)xw[1] + 0.5) * 2.3283064365386962890625e-10;
                             if (__dmul_rn(u, ldg_f64(elem_ptr(a_all, wbase + (uint32_t)p))) < ldg_f64(elem_ptr(a_all, wbase + (uint32_t)c))) p = c;
@@ -151,7 +173,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                         s = sraw + (sraw >= p ? 1 : 0);
                         for (int l = 0; l < P.walk_len; ++l) {
                             uint32_t xw[4];
-                            philox4x32_10((uint32_t)w, sw, mv, (uint32_t)(2 + l), P.seed_lo, P.seed_hi, xw);
+                            walk_words(l, xw);
                             int c = (int)__umulhi(xw[2], (uint32_t)(n_omega - 1));
                             c += (c >= p) ? 1 : 0;
                             const double u = ((double)xw[3] + 0.5) * 2.3283064365386962890625e-10;
@@ -530,7 +552,7 @@ template <int C, int MAXW, bool FACT, bool TRACE, int MODE, int DMMA = 0>
 static int launch_variant(sail_handle *h, SweepArgs &args)
 {
     constexpr int G = 32;
-    constexpr int rec_bytes = (MODE == 2 || MODE == 3) ? kRecMaskBytes : kRecBytes;
+    constexpr int rec_bytes = (MODE == 2 || MODE == 3) ? kRecMaskBytes : (MODE == 4) ? 96 : kRecBytes;
     args.n_groups = args.W;
     int warps = (int)((args.n_groups + h->num_sms - 1) / h->num_sms);
     if (warps > MAXW) warps = MAXW;
