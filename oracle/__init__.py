@@ -33,7 +33,7 @@ class _Problem(C.Structure):
                 ("omega", C.c_void_p), ("K", C.c_void_p), ("F", C.c_void_p), ("sigma", C.c_void_p),
                 ("A", C.c_double), ("B", C.c_double), ("eta", C.c_double),
                 ("amp_mode", C.c_int32), ("amp_p", C.c_double), ("amp_m", C.c_double),
-                ("y_min", C.c_double), ("seed_lo", C.c_uint32), ("seed_hi", C.c_uint32), ("walk_len", C.c_int32)]
+                ("y_min", C.c_double), ("seed_lo", C.c_uint32), ("seed_hi", C.c_uint32), ("walk_len", C.c_int32), ("walk_uniform", C.c_double)]
 
 
 TRACE_DTYPE = np.dtype([("p", "<i4"), ("s", "<i4"), ("flags", "<i4"), ("move", "<i4"),
@@ -147,14 +147,14 @@ class Oracle:
     """State of W walkers + the problem; methods follow include/sail.h call for call."""
 
     def __init__(self, omega, tau, F, sigma, A, B, eta, seed, amp_mode=1, amp_p=1.0, amp_m=2.0,
-                 y_min=1e-6, walk_len=0):
+                 y_min=1e-6, walk_len=0, walk_uniform=0.0):
         self.omega, self.tau, self.F = _f64(omega), _f64(tau), _f64(F)
         self.sigma = _f64(sigma) if sigma is not None else np.ones_like(self.F)
         self.K = kernel_table(self.omega, self.tau)
         self.n_omega, self.n_tau = self.omega.size, self.tau.size
         self.P = _Problem(self.n_omega, self.n_tau, self.omega.ctypes.data, self.K.ctypes.data,
                           self.F.ctypes.data, self.sigma.ctypes.data, A, B, eta, amp_mode, amp_p,
-                          amp_m, y_min, seed & 0xFFFFFFFF, (seed >> 32) & 0xFFFFFFFF, walk_len)
+                          amp_m, y_min, seed & 0xFFFFFFFF, (seed >> 32) & 0xFFFFFFFF, walk_len, walk_uniform)
         self.A, self.B = A, B
         self.sweep = 0
         self.W = 0

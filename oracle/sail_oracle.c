@@ -171,6 +171,8 @@ typedef struct {
     double y_min;          /* floor of y (reading G7)                          */
     uint32_t seed_lo, seed_hi;
     int32_t walk_len;      /* length L of the index-selection walk (section 2.3); 0 = uniform p, s (reading G11) */
+    double walk_uniform;   /* fraction of moves that keep the uniform choice although L > 0 (:158 "a small fraction of
+                            * the uniform distribution can be mixed in")                                            */
 } orc_problem;
 
 /* One traced move (what the parity tests compare). */
@@ -215,14 +217,22 @@ int orc_move(const orc_problem *P, int64_t walker, int64_t sweep, int32_t move, 
      * Metropolis on the bin index with uniform candidates: j <- c if u a_j < a_c.  Step l = 0 .. L-1 draws
      * Philox(ctr = (walker, sweep, move, 2 + l)) = (candidate for p, u for p, candidate for s, u for s); the whole
      * p-walk runs first, then s starts from its uniform draw on the bins other than the final p and walks on those. */
-    for (int l = 0; l < P->walk_len; ++l) {
+    /* the admixture: one more uniform, word 0 of Philox(ctr = (walker, sweep, move, 2 + L)); below walk_uniform the
+     * move keeps its uniform indices */
+    int walk_len = P->walk_len;
+    if (walk_len > 0 && P->walk_uniform > 0.0) {
+        uint32_t cm[4] = { (uint32_t)walker, (uint32_t)sweep, (uint32_t)move, (uint32_t)(2 + P->walk_len) }, xm[4];
+        orc_philox4x32_10(cm, key, xm);
+        if (orc_u01(xm[0]) < P->walk_uniform) walk_len = 0;
+    }
+    for (int l = 0; l < walk_len; ++l) {
         uint32_t cw[4] = { (uint32_t)walker, (uint32_t)sweep, (uint32_t)move, (uint32_t)(2 + l) }, xw[4];
         orc_philox4x32_10(cw, key, xw);
         int32_t c = (int32_t)(((uint64_t)xw[0] * (uint64_t)n_omega) >> 32);
         if (orc_u01(xw[1]) * a[p] < a[c]) p = c;
     }
     if (s >= p) s += 1;
-    for (int l = 0; l < P->walk_len; ++l) {
+    for (int l = 0; l < walk_len; ++l) {
         uint32_t cw[4] = { (uint32_t)walker, (uint32_t)sweep, (uint32_t)move, (uint32_t)(2 + l) }, xw[4];
         orc_philox4x32_10(cw, key, xw);
         int32_t c = (int32_t)(((uint64_t)xw[2] * (uint64_t)(n_omega - 1)) >> 32);

@@ -633,3 +633,27 @@ def test_index_walk_one_step_is_the_metropolis_rule_on_a(tiny):
         assert ps0[m, 0] == p0 and ps1[m, 0] == p1
         moved += p1 != p0
     assert 20 < moved < 190
+
+
+def test_index_walk_uniform_admixture(tiny):
+    """:158 'a small fraction of the uniform distribution can be mixed in': with walk_uniform = f a fraction f of the
+    moves keeps exactly the indices of the zero-length walk, the others exactly those of the pure walk."""
+    N = tiny.n_omega
+    a = np.random.default_rng(11).random(N) ** 4 + 1e-3
+    n = 1500
+    ps0 = _selected_indices(_mk(tiny, 0, 0.0), a, n)
+    psw = _selected_indices(_mk(tiny, 5, 0.0), a, n)
+    psm = _selected_indices(_mk(tiny, 5, 0.3), a, n)
+    same_as_uniform = (psm == ps0).all(axis=1)
+    same_as_walk = (psm == psw).all(axis=1)
+    assert (same_as_uniform | same_as_walk).all()
+    differs = ~(ps0 == psw).all(axis=1)
+    frac = same_as_uniform[differs].mean()
+    assert abs(frac - 0.3) < 4 * np.sqrt(0.3 * 0.7 / differs.sum())
+    np.testing.assert_array_equal(_selected_indices(_mk(tiny, 5, 1.0), a, 200), ps0[:200])
+
+
+def _mk(w, L, f):
+    o = oracle.Oracle(w.omega, w.tau, w.F, w.sigma, w.A, w.B, w.eta, 1234, walk_len=L, walk_uniform=f)
+    o.init_walkers(1)
+    return o
