@@ -125,6 +125,8 @@ typedef struct {
                               * current spectrum (j <- uniform candidate c if u a_j < a_c); 0 = uniform p, s.  The
                               * proposal then depends on the state, so the plain (unscreened) kernel runs it.   */
     int32_t reserved;
+    double  walk_uniform;    /* :158 "a small fraction of the uniform distribution can be mixed in": this fraction
+                              * of the moves keeps its uniform p, s although walk_length > 0; in [0, 1]              */
 } sail_anneal_params;
 
 /*

@@ -36,7 +36,8 @@ class sail_anneal_params(C.Structure):
     _fields_ = [("eta", C.c_double), ("amp_mode", C.c_int32), ("lanes_per_walker", C.c_int32),
                 ("amp_p", C.c_double), ("amp_m", C.c_double), ("y_min", C.c_double),
                 ("resync_every", C.c_int64), ("trace_lo", C.c_int64), ("trace_hi", C.c_int64),
-                ("trace", C.c_void_p), ("flags", C.c_void_p), ("walk_length", C.c_int32), ("reserved", C.c_int32)]
+                ("trace", C.c_void_p), ("flags", C.c_void_p), ("walk_length", C.c_int32), ("reserved", C.c_int32),
+                ("walk_uniform", C.c_double)]
 
 
 class sail_selfcool_params(C.Structure):
@@ -174,14 +175,14 @@ class Sail:
         self.W = W
 
     def anneal(self, T_schedule, eta, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6, resync_every=0,
-               lanes_per_walker=0, trace_walkers=None, want_flags=False, walk_length=0):
+               lanes_per_walker=0, trace_walkers=None, want_flags=False, walk_length=0, walk_uniform=0.0):
         """Run len(T_schedule) sweeps.  Returns (trace, flags) numpy arrays when requested, else (None, None)."""
         import torch
         T = _f64(T_schedule)
         p = sail_anneal_params()
         p.eta, p.amp_mode, p.lanes_per_walker = eta, amp_mode, lanes_per_walker
         p.amp_p, p.amp_m, p.y_min, p.resync_every = amp_p, amp_m, y_min, resync_every
-        p.walk_length = walk_length
+        p.walk_length, p.walk_uniform = walk_length, walk_uniform
         trace_t = flags_t = None
         if trace_walkers is not None:
             lo, hi = trace_walkers

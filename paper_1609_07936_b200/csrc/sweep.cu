@@ -155,6 +155,13 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                         const uint32_t sw = (uint32_t)(P.sweep0 + isw);
                         int p = r0.x, s = r0.y;
                         const int sraw = s - (s > p ? 1 : 0);
+                        // :158 uniform admixture: below walk_uniform the move keeps its uniform indices
+                        int wl = P.walk_len;
+                        if (P.walk_uniform > 0.0) {
+                            uint32_t xm[4];
+                            philox4x32_10((uint32_t)w, sw, mv, (uint32_t)(2 + P.walk_len), P.seed_lo, P.seed_hi, xm);
+                            if (((double)xm[0] + 0.5) * 2.3283064365386962890625e-10 < P.walk_uniform) wl = 0;
+                        }
                         auto walk_words = [&](int l, uint32_t (&xw)[4]) {
                             if (l < 2) {
                                 const int4 q = lds_s32x4(r + 64 + 16 * l);
@@ -163,7 +170,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                                 philox4x32_10((uint32_t)w, sw, mv, (uint32_t)(2 + l), P.seed_lo, P.seed_hi, xw);
                             }
                         };
-                        for (int l = 0; l < P.walk_len; ++l) {
+                        for (int l = 0; l < wl; ++l) {
                             uint32_t xw[4];
                             walk_words(l, xw);
                             const int c = (int)__umulhi(xw[0], (uint32_t)n_omega);
@@ -171,7 +178,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                             if (__dmul_rn(u, ldg_f64(elem_ptr(a_all, wbase + (uint32_t)p))) < ldg_f64(elem_ptr(a_all, wbase + (uint32_t)c))) p = c;
                         }
                         s = sraw + (sraw >= p ? 1 : 0);
-                        for (int l = 0; l < P.walk_len; ++l) {
+                        for (int l = 0; l < wl; ++l) {
                             uint32_t xw[4];
                             walk_words(l, xw);
                             int c = (int)__umulhi(xw[2], (uint32_t)(n_omega - 1));
@@ -596,6 +603,7 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     if (!(req == 0 || req == 8 || req == 16 || req == 32 || (req >= 34 && req <= 37)))
         return set_err(h, SAIL_ERR_ARG, "lanes_per_walker=%d is not one of 0, 8, 16, 32, 34..37", req);
     if (p->walk_length < 0 || p->walk_length > 4096) return set_err(h, SAIL_ERR_ARG, "walk_length=%d outside [0, 4096]", p->walk_length);
+    if (!(p->walk_uniform >= 0.0 && p->walk_uniform <= 1.0)) return set_err(h, SAIL_ERR_ARG, "walk_uniform must lie in [0, 1]");
     if (p->walk_length > 0 && !(req == 0 || req == 32 || req == 34))
         return set_err(h, SAIL_ERR_ARG, "walk_length > 0 runs on the plain one-walker-per-warp kernel: lanes_per_walker must be 0, 32 or 34");
     const int G = pick_lanes(req);
@@ -625,7 +633,7 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
     a.a = h->st.a; a.mt = h->st.mt; a.chi2 = h->st.chi2; a.y = h->st.y;
     a.n_acc = h->st.n_acc; a.n_eval = h->st.n_eval;
     a.T = d_T; a.sweep0 = h->sweep; a.n_sweeps = (int)n_sweeps;
-    a.walk_len = p->walk_length;
+    a.walk_len = p->walk_length; a.walk_uniform = p->walk_uniform;
     a.trace_lo = p->trace_lo; a.trace_hi = p->trace_hi; a.trace = p->trace; a.flags = p->flags;
     a.call_sweeps = sweeps_in_call; a.call_off = call_offset;
     const bool trace = (p->trace != nullptr) || (p->flags != nullptr);

@@ -19,6 +19,7 @@ struct SweepArgs {
     long long sweep0;
     int n_sweeps;
     int walk_len;                      // length of the index-selection walk (section 2.3); 0 = uniform indices
+    double walk_uniform;               // fraction of moves that keep the uniform indices (:158)
     long long trace_lo, trace_hi;
     sail_trace_rec *trace;
     uint8_t *flags;

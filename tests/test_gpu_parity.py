@@ -600,17 +600,18 @@ def test_schedule_longer_than_the_device_slice_is_uploaded_in_pieces():
     s1.close(); s2.close()
 
 
-@pytest.mark.parametrize("name,W,L,n_sw", [("tiny", 64, 1, 20), ("tiny", 64, 3, 20), ("small", 45, 2, 6), ("stress", 9, 2, 2)])
-def test_index_walk_parity(name, W, L, n_sw):
+@pytest.mark.parametrize("name,W,L,n_sw,mix", [("tiny", 64, 1, 20, 0.0), ("tiny", 64, 3, 20, 0.25), ("small", 45, 2, 6, 0.0),
+                                               ("stress", 9, 2, 2, 0.1)])
+def test_index_walk_parity(name, W, L, n_sw, mix):
     """f4 (section 2.3, :156-158; reading F4): with p and s chosen by an L-step Metropolis walk on the CURRENT spectrum
     the GPU still makes the oracle's moves one for one: identical indices, rho, decisions; dchi2 within 1e-12 L1."""
     w = wl.make(name, simpson_intervals=20_000)
-    o = oracle.Oracle(w.omega, w.tau, w.F, w.sigma, w.A, w.B, w.eta, SEED, walk_len=L)
+    o = oracle.Oracle(w.omega, w.tau, w.F, w.sigma, w.A, w.B, w.eta, SEED, walk_len=L, walk_uniform=mix)
     o.init_walkers(W)
     s = _sail(w, W)
     s.init_walkers(W, w.A, w.B, SEED, spectra=o.a)
     T = wl.geometric_schedule(1.0, 0.3, n_sw)
-    tg, fg = s.anneal(T, w.eta, trace_walkers=(0, W), want_flags=True, walk_length=L)
+    tg, fg = s.anneal(T, w.eta, trace_walkers=(0, W), want_flags=True, walk_length=L, walk_uniform=mix)
     to, fo = o.anneal(T, trace_walkers=(0, W), want_flags=True)
     assert compare_traces(tg, to, T, w.A / w.n_omega) == 0
     assert ((fg & 3) == fo).all()
