@@ -177,6 +177,35 @@ def main_reference(args):
     return 0
 
 
+def main_selfcool(args):
+    """Supplementary: the paper's own protocol (self-cooling, blocks of 100 sweeps, smoothing, a quarter of the walkers
+    branched with t = 0.1, strength following the acceptance rate) on the chosen workload; prints the trajectory."""
+    import torch
+    from paper_1609_07936_b200 import build
+    build.build()
+    from paper_1609_07936_b200.binding import Sail
+    w = wl.make(args.workload)
+    s = Sail(w.omega, w.tau, w.F, w.sigma, max_walkers=w.W)
+    s.init_walkers(w.W, w.A, w.B, w.rng_seed)
+    nb, k = args.selfcool, 100
+    kw = dict(n_boil=max(1, nb // 10), n_ramp=max(1, nb // 5), eta=w.eta, t_imprint=0.1, smooth_s=0.01, branch_fraction=0.25,
+              adapt=True, freeze_rate=0.5)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    T, ave, mn = s.anneal_selfcool(nb, k, **kw)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    mn_end, ave_end = s.chi2_stats()
+    acc, ev, _ = s.stats()
+    print(json.dumps({"protocol": "self-cooling (sail_anneal_selfcool)", "workload": w.name, "blocks": nb, "sweeps_per_block": k,
+                      "parameters": {a: b for a, b in kw.items() if a != "eta"}, "seconds": dt,
+                      "attempted_moves_per_s": w.W * nb * k * w.n_omega / dt, "accepted_fraction": float(acc.sum()) / (w.W * nb * k * w.n_omega),
+                      "T": [float(x) for x in T], "chi2_ave": [float(x) for x in ave], "chi2_min": [float(x) for x in mn],
+                      "chi2_ave_end": ave_end, "chi2_min_end": mn_end, "n_tau": w.n_tau}))
+    s.close()
+    return 0
+
+
 def main_ours(args):
     import torch
     if not torch.cuda.is_available():
@@ -403,6 +432,9 @@ if __name__ == "__main__":
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--extra", type=int, default=1, help="also time a block of the stress config (N=1 only)")
     ap.add_argument("--lanes", type=int, default=0, help="lanes per walker / kernel form: 0 auto, 8, 16, 32..35 (include/sail.h)")
+    ap.add_argument("--selfcool", type=int, default=0, help="run N blocks of the paper's self-cooling protocol instead of the bench (supplementary)")
     a = ap.parse_args()
     LANES = a.lanes
+    if a.selfcool > 0 and a.impl == "ours":
+        sys.exit(main_selfcool(a))
     sys.exit(main_reference(a) if a.impl == "reference" else main_ours(a))
