@@ -105,3 +105,14 @@ def test_product_does_not_import_the_oracle():
     otext = open(os.path.join(ROOT, "oracle", "__init__.py")).read() + open(os.path.join(ROOT, "oracle", "sail_oracle.c")).read()
     assert "import paper_1609_07936_b200" not in otext and "from paper_1609_07936_b200" not in otext
     assert "sail.h" not in otext.replace("include/sail.h", "")
+
+
+def test_header_is_plain_c(tmp_path):
+    """include/sail.h must compile as C99 (the boundary is a C ABI: no C++ or torch types in the signatures)."""
+    import subprocess
+    src = tmp_path / "t.c"
+    src.write_text('#include "sail.h"\nint main(void) { sail_anneal_params p; sail_selfcool_params q; sail_branch_info i;\n'
+                   '  (void)p; (void)q; (void)i; return SAIL_MICROBENCH_N; }\n')
+    r = subprocess.run(["gcc", "-std=c99", "-Wall", "-Wextra", "-Werror", "-fsyntax-only", "-I", os.path.join(ROOT, "include"), str(src)],
+                       capture_output=True, text=True)
+    assert r.returncode == 0, r.stderr
