@@ -98,12 +98,9 @@ def measured_peaks():
 # (profiles/r01_sweep_small_full_metrics.txt): 12.06 MB + 3.07 MB for the whole 5000-sweep Small anneal
 SWEEP_DRAM_BYTES_PER_LAUNCH = {("small", 5000): 15.13e6}
 
-LANES = 0   # --lanes: lanes of a warp per walker (0 = library default)
-
 
 def anneal_params(w):
-    return dict(eta=w.eta, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6, resync_every=w.resync_every,
-                lanes_per_walker=LANES)
+    return dict(eta=w.eta, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6, resync_every=w.resync_every)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -431,10 +428,8 @@ if __name__ == "__main__":
     ap.add_argument("--sweeps", type=int, default=0, help="override the number of sweeps (debug)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
     ap.add_argument("--extra", type=int, default=1, help="also time a block of the stress config (N=1 only)")
-    ap.add_argument("--lanes", type=int, default=0, help="lanes per walker / kernel form: 0 auto, 8, 16, 32..35 (include/sail.h)")
     ap.add_argument("--selfcool", type=int, default=0, help="run N blocks of the paper's self-cooling protocol instead of the bench (supplementary)")
     a = ap.parse_args()
-    LANES = a.lanes
     if a.selfcool > 0 and a.impl == "ours":
         sys.exit(main_selfcool(a))
     sys.exit(main_reference(a) if a.impl == "reference" else main_ours(a))

@@ -74,7 +74,9 @@ SAIL_API size_t sail_workspace_bytes(int32_t n_omega, int32_t n_tau, int64_t max
  *   F      HOST [n_tau]    correlation data F~(tau_j)
  *   sigma  HOST [n_tau]    error bars > 0, or NULL for sigma = 1 (the paper's unweighted Eq. 9)
  * Inputs are copied; the caller keeps ownership.  Builds the device tables (c_j, exp(-omega_k tau_j),
- * weights (c_j/sigma_j)^2).  Limits of this version: 2 <= n_omega <= 8192, 1 <= n_tau <= 512.
+ * weights (c_j/sigma_j)^2).  Limits of this version: 2 <= n_omega <= 8192 (the sweep kernel keeps two n_omega-sized
+ * tables and the start table in the 227 KB of shared memory of an SM; it runs fewer warps per SM above ~4000 bins),
+ * 1 <= n_tau <= 512 (16 tau-points per lane in registers); sail_smooth needs n_omega <= 2048.
  * Errors: SAIL_ERR_ARG, SAIL_ERR_GRID (the method is defined on uniform grids only, Eq. 2-3, 7),
  * SAIL_ERR_ALLOC, SAIL_ERR_CUDA.  *out is NULL on error.
  */
@@ -110,11 +112,7 @@ typedef struct {
 typedef struct {
     double  eta;             /* base amplitude: rho = 1 - y eta (2u - 1), requires 0 < eta < 1 (reading G6) */
     int32_t amp_mode;        /* 0: y = 1;  1: Eq. 30 from the previous sweep's acceptance  */
-    int32_t lanes_per_walker;/* sweep-kernel form, a tuning knob (all forms make the same moves and decisions):
-                              * 0 / 32 screened one-walker-per-warp kernel, DMMA warp sum (default);
-                              * 37 the same with the shuffle butterfly; 35 the same, other register budget;
-                              * 34 unscreened form; 8 / 16 lanes per walker: several walkers per warp in
-                              * lockstep; 36 the 32-lane instance of that kernel          */
+    int32_t reserved0;       /* must be 0 (there is one sweep-kernel form: DESIGN.md 6.1)                 */
     double  amp_p, amp_m;    /* Eq. 30 parameters (paper: p = 1, m = 2, :222)                      */
     double  y_min;           /* floor of y (reading G7), e.g. 1e-6                                  */
     int64_t resync_every;    /* full-residual resync after every such absolute sweep; 0 = never    */
@@ -122,8 +120,8 @@ typedef struct {
     sail_trace_rec *trace;   /* DEVICE [(hi-lo)][n_sweeps][n_omega] or NULL                        */
     uint8_t *flags;          /* DEVICE [W][n_sweeps][n_omega] per-move flag bytes, or NULL         */
     int32_t walk_length;     /* section 2.3 (:156-158): p and s by a truncated Markov walk of this many steps on the
-                              * current spectrum (j <- uniform candidate c if u a_j < a_c); 0 = uniform p, s.  The
-                              * proposal then depends on the state, so the plain (unscreened) kernel runs it.   */
+                              * current spectrum (j <- uniform candidate c if u a_j < a_c); 0 = uniform p, s.  Every
+                              * lane of the batch walks its own move; the moves behind an accepted one walk again.   */
     int32_t reserved;
     double  walk_uniform;    /* :158 "a small fraction of the uniform distribution can be mixed in": this fraction
                               * of the moves keeps its uniform p, s although walk_length > 0; in [0, 1]              */

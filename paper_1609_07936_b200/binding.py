@@ -33,7 +33,7 @@ class sail_config(C.Structure):
 
 
 class sail_anneal_params(C.Structure):
-    _fields_ = [("eta", C.c_double), ("amp_mode", C.c_int32), ("lanes_per_walker", C.c_int32),
+    _fields_ = [("eta", C.c_double), ("amp_mode", C.c_int32), ("reserved0", C.c_int32),
                 ("amp_p", C.c_double), ("amp_m", C.c_double), ("y_min", C.c_double),
                 ("resync_every", C.c_int64), ("trace_lo", C.c_int64), ("trace_hi", C.c_int64),
                 ("trace", C.c_void_p), ("flags", C.c_void_p), ("walk_length", C.c_int32), ("reserved", C.c_int32),
@@ -175,12 +175,12 @@ class Sail:
         self.W = W
 
     def anneal(self, T_schedule, eta, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6, resync_every=0,
-               lanes_per_walker=0, trace_walkers=None, want_flags=False, walk_length=0, walk_uniform=0.0):
+               trace_walkers=None, want_flags=False, walk_length=0, walk_uniform=0.0):
         """Run len(T_schedule) sweeps.  Returns (trace, flags) numpy arrays when requested, else (None, None)."""
         import torch
         T = _f64(T_schedule)
         p = sail_anneal_params()
-        p.eta, p.amp_mode, p.lanes_per_walker = eta, amp_mode, lanes_per_walker
+        p.eta, p.amp_mode = eta, amp_mode
         p.amp_p, p.amp_m, p.y_min, p.resync_every = amp_p, amp_m, y_min, resync_every
         p.walk_length, p.walk_uniform = walk_length, walk_uniform
         trace_t = flags_t = None
@@ -209,8 +209,7 @@ class Sail:
         return mn.value, mean.value
 
     def anneal_selfcool(self, n_blocks, sweeps_per_block, n_boil, n_ramp, eta, t_imprint=0.1, smooth_s=0.0, T_start=10.0,
-                        freeze_rate=1.0, branch=True, branch_fraction=0.0, adapt=False, T_override=None, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6,
-                        lanes_per_walker=0):
+                        freeze_rate=1.0, branch=True, branch_fraction=0.0, adapt=False, T_override=None, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6):
         """The paper's block protocol with self-cooling (include/sail.h: sail_anneal_selfcool).
         Returns (T, chi2_ave, chi2_min), one entry per block."""
         p = sail_selfcool_params()
@@ -220,7 +219,7 @@ class Sail:
         p.adapt = int(adapt)
         ov = _f64(T_override) if T_override is not None else None
         p.T_override = ov.ctypes.data if ov is not None else None
-        p.anneal.eta, p.anneal.amp_mode, p.anneal.lanes_per_walker = eta, amp_mode, lanes_per_walker
+        p.anneal.eta, p.anneal.amp_mode = eta, amp_mode
         p.anneal.amp_p, p.anneal.amp_m, p.anneal.y_min = amp_p, amp_m, y_min
         T, ave, mn = np.zeros(n_blocks), np.zeros(n_blocks), np.zeros(n_blocks)
         self._check(self._L.sail_anneal_selfcool(self._h, C.byref(p), n_blocks, _ptr(T), _ptr(ave), _ptr(mn)))

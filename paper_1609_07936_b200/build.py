@@ -16,7 +16,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libsail_b200.so")
 INCLUDE = os.path.join(os.path.dirname(HERE), "include")
-SOURCES = ["sail_api.cu", "sweep.cu", "sweep_grp.cu", "forward.cu", "branch.cu", "smooth.cu", "selfcool.cu", "microbench.cu"]
+SOURCES = ["sail_api.cu", "sweep.cu", "forward.cu", "branch.cu", "smooth.cu", "selfcool.cu", "microbench.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]
 

@@ -11,12 +11,24 @@ constexpr int kScanThreads = 256;
 constexpr int kScanItems = 4;
 constexpr int kScanTile = kScanThreads * kScanItems;   // 1024 elements per CTA
 
+// Order-preserving key of a double: the running residue chi2_0 + sum dchi2 can dip below zero near an exact fit, so
+// the plain bit pattern (valid for values >= 0 only) is not enough.  Negative values have all bits flipped, the others
+// only the sign bit: unsigned comparison of keys orders like the values (-0 < +0, NaN above +inf).
+__device__ __forceinline__ unsigned long long ordered_key(double v)
+{
+    const unsigned long long b = (unsigned long long)__double_as_longlong(v);
+    return (b >> 63) ? ~b : (b | 0x8000000000000000ull);
+}
+__device__ __forceinline__ double key_value(unsigned long long k)
+{
+    return __longlong_as_double((long long)((k >> 63) ? (k & 0x7fffffffffffffffull) : ~k));
+}
+
 __global__ void chi2_min_kernel(long long W, const double *__restrict__ chi2, unsigned long long *scalars)
 {
-    // chi^2 >= 0, so the IEEE bit patterns order like the values
     unsigned long long m = ~0ull;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
-        const unsigned long long b = (unsigned long long)__double_as_longlong(chi2[i]);
+        const unsigned long long b = ordered_key(chi2[i]);
         m = b < m ? b : m;
     }
 #pragma unroll
@@ -31,10 +43,11 @@ __global__ void chi2_min_kernel(long long W, const double *__restrict__ chi2, un
 __global__ void weights_kernel(long long W, const double *__restrict__ chi2, double T,
                                const unsigned long long *scalars, unsigned long long *ehat)
 {
-    const double cmin = __longlong_as_double((long long)scalars[0]);
+    const double cmin = key_value(scalars[0]);
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
+        // chi2_i >= chi2_min makes the exponent <= 0 and the weight <= 2^40; a NaN residue gets weight 0
         const double e = exp(-(chi2[i] - cmin) / T);
-        ehat[i] = (unsigned long long)floor(e * 1099511627776.0);
+        ehat[i] = (e == e) ? (unsigned long long)floor(fmin(e, 1.0) * 1099511627776.0) : 0ull;
     }
 }
 
@@ -361,7 +374,7 @@ static int branch_imprint(sail_handle *h, double t_imprint)
     const bool copy = t_imprint == 1.0;
     const int nst = copy ? 3 : 2;
     const size_t tma_smem = (copy ? 1 : 2) * row_bytes * nst;
-    if ((h->n_omega & 1) == 0 && (h->n_tau & 1) == 0 && tma_smem <= 96 * 1024 && copy && !h->no_tma_imprint) {
+    if ((h->n_omega & 1) == 0 && (h->n_tau & 1) == 0 && tma_smem <= 96 * 1024 && copy) {
         const int per_sm = (int)((200 * 1024) / (tma_smem + 1024)) < 8 ? (int)((200 * 1024) / (tma_smem + 1024)) : 8;
         const int tblocks = (int)(W < (long long)h->num_sms * per_sm ? W : (long long)h->num_sms * per_sm);
         if (copy) {
@@ -395,9 +408,9 @@ int launch_branch(sail_handle *h, double T, double t_imprint)
 
 __global__ void chi2_max_kernel(long long W, const double *__restrict__ chi2, unsigned long long *dst)
 {
-    unsigned long long m = 0ull;                       // chi^2 >= 0: the bit patterns order like the values
+    unsigned long long m = 0ull;
     for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
-        const unsigned long long b = (unsigned long long)__double_as_longlong(chi2[i]);
+        const unsigned long long b = ordered_key(chi2[i]);
         m = b > m ? b : m;
     }
 #pragma unroll
@@ -428,7 +441,7 @@ int launch_branch_fraction(sail_handle *h, double fraction, double t_imprint, do
     SAIL_CUDA_OK(h, cudaMemcpyAsync(sc, b.scalars, sizeof sc, cudaMemcpyDeviceToHost, h->stream));
     SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
     double cmin, cmax;
-    memcpy(&cmin, &sc[0], 8); memcpy(&cmax, &sc[6], 8);
+    cmin = ordered_key_value(sc[0]); cmax = ordered_key_value(sc[6]);
     if (n0 <= 0 || !(cmax > cmin)) return SAIL_OK;     // nothing to branch
     int rc = SAIL_OK;
     auto zeros = [&](double beta) -> long long {

@@ -28,7 +28,7 @@ int set_err(sail_handle *h, int code, const char *fmt, ...)
 // ---- workspace layout ------------------------------------------------------------------------------
 struct Layout {
     size_t off_omega, off_tau, off_c, off_Wj, off_fj, off_F, off_sigma, off_E, off_ET, off_ratio, off_invd, off_E0, off_T;
-    size_t off_a, off_mt, off_chi2, off_y, off_nacc, off_neval;
+    size_t off_a, off_mt, off_chi2, off_y, off_nacc, off_neval, off_model;
     size_t off_ehat, off_scanA, off_scanB, off_bsums, off_mult, off_donor, off_reclist, off_scalars;
     size_t total;
 };
@@ -40,8 +40,7 @@ static Layout make_layout(int n_omega, int n_tau, int64_t Wmax)
     Layout L{};
     size_t off = 0;
     auto take = [&](size_t bytes) { size_t o = off; off += (bytes + 255) & ~(size_t)255; return o; };
-    // + 3 scratch walker slots: the sweep kernel pads W to a multiple of 4 (see sweep.cu)
-    const size_t W = (size_t)Wmax + 3, d = sizeof(double), u = sizeof(unsigned long long);
+    const size_t W = (size_t)Wmax, d = sizeof(double), u = sizeof(unsigned long long);
     L.off_omega = take(n_omega * d);  L.off_tau = take(n_tau * d);   L.off_c = take(n_tau * d);
     L.off_Wj = take(n_tau * d);       L.off_fj = take(n_tau * d);    L.off_F = take(n_tau * d);
     L.off_sigma = take(n_tau * d);    L.off_E = take((size_t)n_omega * n_tau * d);
@@ -51,6 +50,7 @@ static Layout make_layout(int n_omega, int n_tau, int64_t Wmax)
     L.off_a = take(W * n_omega * d);  L.off_mt = take(W * n_tau * d);
     L.off_chi2 = take(W * d);         L.off_y = take(W * d);
     L.off_nacc = take(W * u);         L.off_neval = take(W * u);
+    L.off_model = take(W * n_tau * d);
     L.off_ehat = take(W * u);         L.off_scanA = take(W * u);     L.off_scanB = take(W * u);
     L.off_bsums = take(3 * ((W + 1023) / 1024 + 1) * u);
     L.off_mult = take(W * sizeof(int32_t));
@@ -157,7 +157,7 @@ int sail_create(sail_t **out, const double *omega, int32_t n_omega, const double
     if (!out) return set_err(nullptr, SAIL_ERR_ARG, "out is NULL");
     *out = nullptr;
     if (!omega || !tau || !F || !cfg) return set_err(nullptr, SAIL_ERR_ARG, "NULL argument");
-    if (n_omega < 2 || n_omega > kMaxOmega) return set_err(nullptr, SAIL_ERR_ARG, "n_omega=%d outside [2, %d]", n_omega, kMaxOmega);
+    if (n_omega < 2 || n_omega > kMaxOmega || !sweep_fits(n_omega)) return set_err(nullptr, SAIL_ERR_ARG, "n_omega=%d outside [2, %d]", n_omega, kMaxOmega);
     if (n_tau < 1 || n_tau > kMaxTau) return set_err(nullptr, SAIL_ERR_ARG, "n_tau=%d outside [1, %d]", n_tau, kMaxTau);
     if (cfg->max_walkers < 1) return set_err(nullptr, SAIL_ERR_ARG, "max_walkers < 1");
     double w0, dw, t0, dt;
@@ -182,6 +182,7 @@ int sail_create(sail_t **out, const double *omega, int32_t n_omega, const double
     h->stream = (cudaStream_t)cfg->stream;
     h->n_omega = n_omega; h->n_tau = n_tau; h->max_walkers = cfg->max_walkers;
     h->omega0 = w0; h->domega = dw; h->tau0 = t0; h->dtau = dt;
+    h->omega_host.assign(omega, omega + n_omega);         // the start spectrum (reading G4) is a host-side bisection on the grid
 
     const Layout L = make_layout(n_omega, n_tau, cfg->max_walkers);
     if (cfg->workspace) {
@@ -201,7 +202,7 @@ int sail_create(sail_t **out, const double *omega, int32_t n_omega, const double
     h->sw_ratio = D(L.off_ratio); h->sw_invd = D(L.off_invd); h->sw_E0 = D(L.off_E0);
     h->d_T = D(L.off_T); h->d_T_cap = kScheduleDoubles;
     h->st.a = D(L.off_a); h->st.mt = D(L.off_mt); h->st.chi2 = D(L.off_chi2); h->st.y = D(L.off_y);
-    h->st.n_acc = U(L.off_nacc); h->st.n_eval = U(L.off_neval);
+    h->st.n_acc = U(L.off_nacc); h->st.n_eval = U(L.off_neval); h->model_scratch = D(L.off_model);
     h->br.ehat = U(L.off_ehat); h->br.scanA = U(L.off_scanA); h->br.scanB = U(L.off_scanB);
     h->br.block_sums = U(L.off_bsums); h->br.mult = (int32_t *)(base + L.off_mult);
     h->br.donor_of = (int64_t *)(base + L.off_donor); h->br.rec_list = (int64_t *)(base + L.off_reclist);
@@ -215,7 +216,6 @@ int sail_create(sail_t **out, const double *omega, int32_t n_omega, const double
     rc = launch_problem_tables(h, D(L.off_F), sigma ? D(L.off_sigma) : nullptr, D(L.off_c), D(L.off_Wj), D(L.off_fj), D(L.off_E));
     if (rc) return fail(rc);
     if (cudaStreamSynchronize(h->stream) != cudaSuccess) return fail(set_err(h, SAIL_ERR_CUDA, "table build failed: %s", cudaGetErrorString(cudaGetLastError())));
-    h->no_tma_imprint = getenv("SAIL_NO_TMA_IMPRINT") != nullptr;
     *out = h;
     return SAIL_OK;
 }
@@ -227,28 +227,32 @@ int sail_init_walkers(sail_t *h, int64_t W, double A, double B, uint64_t seed, i
     if (!(A > 0.0) || !isfinite(B)) return set_err(h, SAIL_ERR_ARG, "A must be > 0 and B finite");
     if (mode != 0 && mode != 1) return set_err(h, SAIL_ERR_ARG, "mode must be 0 or 1");
     SAIL_CUDA_OK(h, cudaSetDevice(h->device));
-    h->W = W; h->A = A; h->B = B; h->seed = seed; h->sweep = 0;
-    const int blocks = (int)((W + 255) / 256 < 2048 ? (W + 255) / 256 : 2048);
+    // everything that can be refused is checked before the handle changes: a failed re-initialisation leaves the
+    // previous population and its constants intact
+    std::vector<double> tilt;
     if (mode == 0) {
-        std::vector<double> omega(h->n_omega), a;
-        SAIL_CUDA_OK(h, cudaMemcpyAsync(omega.data(), h->tab.omega, h->n_omega * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-        SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
-        if (!tilt_spectrum(h, omega, A, B, a)) return set_err(h, SAIL_ERR_ARG, "B/A = %g lies outside the bin midpoints of the omega grid", B / A);
-        SAIL_CUDA_OK(h, cudaMemcpyAsync(h->st.a, a.data(), h->n_omega * sizeof(double), cudaMemcpyHostToDevice, h->stream));
-        SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));   // 'a' is a local vector
-        if (W > 1) {
-            broadcast_rows_kernel<<<2048, 256, 0, h->stream>>>(h->n_omega, W, h->st.a);
-            SAIL_LAUNCH_OK(h, "broadcast_rows_kernel");
-        }
+        if (!tilt_spectrum(h, h->omega_host, A, B, tilt)) return set_err(h, SAIL_ERR_ARG, "B/A = %g lies outside the bin midpoints of the omega grid", B / A);
     } else {
         if (!spectra) return set_err(h, SAIL_ERR_ARG, "mode 1 needs spectra");
         const size_t n = (size_t)W * h->n_omega;
         for (size_t i = 0; i < n; ++i)
             if (!(spectra[i] >= 0.0)) return set_err(h, SAIL_ERR_ARG, "spectra[%zu] is negative or NaN", i);
-        SAIL_CUDA_OK(h, cudaMemcpyAsync(h->st.a, spectra, n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
     }
-    fill_state_kernel<<<blocks, 256, 0, h->stream>>>(W + 3, h->st.y, h->st.n_acc, h->st.n_eval);
+    h->initialised = false;                       // from here on the device state is being rewritten
+    const int blocks = (int)((W + 255) / 256 < 2048 ? (W + 255) / 256 : 2048);
+    if (mode == 0) {
+        SAIL_CUDA_OK(h, cudaMemcpyAsync(h->st.a, tilt.data(), h->n_omega * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+        SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));   // 'tilt' is a local vector
+        if (W > 1) {
+            broadcast_rows_kernel<<<2048, 256, 0, h->stream>>>(h->n_omega, W, h->st.a);
+            SAIL_LAUNCH_OK(h, "broadcast_rows_kernel");
+        }
+    } else {
+        SAIL_CUDA_OK(h, cudaMemcpyAsync(h->st.a, spectra, (size_t)W * h->n_omega * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    }
+    fill_state_kernel<<<blocks, 256, 0, h->stream>>>(W, h->st.y, h->st.n_acc, h->st.n_eval);
     SAIL_LAUNCH_OK(h, "fill_state_kernel");
+    h->W = W; h->A = A; h->B = B; h->seed = seed; h->sweep = 0;
     int rc = launch_forward(h, 0, W);
     if (rc) return rc;
     SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
@@ -268,6 +272,7 @@ int sail_anneal(sail_t *h, const double *T_schedule, int64_t n_sweeps, const sai
     if (p->trace && !(p->trace_lo >= 0 && p->trace_lo <= p->trace_hi && p->trace_hi <= h->W))
         return set_err(h, SAIL_ERR_ARG, "trace range outside [0, W]");
     if (p->resync_every < 0) return set_err(h, SAIL_ERR_ARG, "resync_every < 0");
+    if (p->reserved0 != 0 || p->reserved != 0) return set_err(h, SAIL_ERR_ARG, "reserved fields of sail_anneal_params must be 0");
     for (int64_t i = 0; i < n_sweeps; ++i)
         if (!(T_schedule[i] > 0.0)) return set_err(h, SAIL_ERR_ARG, "T_schedule[%lld] must be > 0", (long long)i);
     if (n_sweeps == 0) return SAIL_OK;
@@ -309,9 +314,7 @@ static int branch_outputs(sail_t *h, sail_branch_info *info, int32_t *mult_out, 
         if (donor_out) SAIL_CUDA_OK(h, cudaMemcpyAsync(donor_out, h->br.donor_of, h->W * sizeof(int64_t), cudaMemcpyDeviceToHost, h->stream));
         SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
         if (info) {
-            double cmin;
-            memcpy(&cmin, &sc[0], sizeof cmin);
-            info->chi2_min = cmin;
+            info->chi2_min = ordered_key_value(sc[0]);
             info->n_recipients = (int64_t)sc[2];
             info->max_multiplier = (int32_t)sc[3];
             info->reserved = 0;
@@ -388,16 +391,11 @@ int sail_get_model(sail_t *h, double *M, int32_t on_device)
     SAIL_CUDA_OK(h, cudaSetDevice(h->device));
     const size_t bytes = (size_t)h->W * h->n_tau * sizeof(double);
     if (on_device) return launch_scale_model(h, M);
-    double *tmp = nullptr;
-    SAIL_CUDA_OK(h, cudaMalloc(&tmp, bytes));
-    int rc = launch_scale_model(h, tmp);
-    if (rc == SAIL_OK) {
-        cudaError_t e = cudaMemcpyAsync(M, tmp, bytes, cudaMemcpyDeviceToHost, h->stream);
-        if (e == cudaSuccess) e = cudaStreamSynchronize(h->stream);
-        if (e != cudaSuccess) rc = set_err(h, SAIL_ERR_CUDA, "copy of model failed: %s", cudaGetErrorString(e));
-    }
-    cudaFree(tmp);
-    return rc;
+    int rc = launch_scale_model(h, h->model_scratch);     // a slice of the workspace: no allocation per call
+    if (rc) return rc;
+    SAIL_CUDA_OK(h, cudaMemcpyAsync(M, h->model_scratch, bytes, cudaMemcpyDeviceToHost, h->stream));
+    SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
+    return SAIL_OK;
 }
 
 int sail_stats(sail_t *h, int64_t *accepted, int64_t *evaluated, double *y)

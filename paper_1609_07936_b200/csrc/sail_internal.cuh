@@ -4,15 +4,16 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 #include <stdio.h>
+#include <string.h>
 #include <string>
+#include <vector>
 
 #include "../../include/sail.h"
 
 namespace sail {
 
 constexpr int kMaxTau = 512;        // 32 lanes x 16 tau-points per lane (register-resident residual)
-constexpr int kMaxOmega = 8192;     // ratio + start tables + proposal records must fit 227 KB of shared memory
-constexpr int kRecBytes = 64;       // one staged proposal record in shared memory
+constexpr int kMaxOmega = 8192;     // sweep-kernel tables (ratio, 1/(k domega), start values) + proposal records fit 227 KB of shared memory
 
 // ------------------------------------------------------------------------------------------------
 // Device-side layout of one handle.  All arrays live in ONE workspace (caller- or library-owned).
@@ -60,6 +61,7 @@ struct sail_handle {
     int64_t max_walkers = 0, W = 0;
     double omega0 = 0, domega = 0, tau0 = 0, dtau = 0;
     double A = 0, B = 0;
+    std::vector<double> omega_host;   // the caller's omega grid (sail_create copies it)
     uint64_t seed = 0;
     int64_t sweep = 0;          // absolute sweep counter
     bool initialised = false;
@@ -71,8 +73,8 @@ struct sail_handle {
     sail::DevTables tab{};
     sail::DevState st{};
     sail::BranchScratch br{};
-    // sweep-kernel tables for the lane count last used (rebuilt when it changes)
-    int tables_G = 0;
+    // sweep-kernel tables (built by the first sail_anneal)
+    bool tables_ready = false;
     bool tables_fact = false;
     int fact_shift = 0;
     double *sw_ratio = nullptr;  // [n_omega] exp(-omega_k G dtau)
@@ -80,10 +82,7 @@ struct sail_handle {
     double *sw_E0 = nullptr;     // direct: [n_omega][G]; factored: H[n_hi][G] then L[n_lo][G]
     double *d_T = nullptr;       // device copy of the schedule piece in flight (a fixed slice of the workspace)
     size_t d_T_cap = 0;
-    double *h_pinned = nullptr;  // small pinned staging buffer
-    size_t h_pinned_cap = 0;
-
-    bool no_tma_imprint = false;   // SAIL_NO_TMA_IMPRINT=1 in the environment at sail_create: plain-load imprint kernel (A/B measurements)
+    double *model_scratch = nullptr;   // [max_walkers][n_tau]: sail_get_model's scaled copy M = c mt for the host
 
     int64_t launches = 0;
     std::string err;
@@ -129,6 +128,15 @@ __host__ __device__ __forceinline__ void philox4x32_10(uint32_t c0, uint32_t c1,
     out[0] = c0; out[1] = c1; out[2] = c2; out[3] = c3;
 }
 
+// order-preserving key of a double as written by the residue min / max kernels (branch.cu), decoded on the host
+inline double ordered_key_value(unsigned long long k)
+{
+    const unsigned long long b = (k >> 63) ? (k & 0x7fffffffffffffffull) : ~k;
+    double v;
+    memcpy(&v, &b, sizeof v);
+    return v;
+}
+
 // ---- entry points implemented in the other translation units ---------------------------------------
 int launch_problem_tables(sail_handle *h, const double *d_F, const double *d_sigma, double *c, double *Wj,
                           double *fj, double *E);
@@ -139,6 +147,7 @@ int launch_branch(sail_handle *h, double T, double t_imprint);
 int launch_branch_fraction(sail_handle *h, double fraction, double t_imprint, double *T_found);   // row f2
 int launch_smooth(sail_handle *h, double s);                          // Eq. 27-29 + renormalisation + forward
 int launch_scale_model(sail_handle *h, double *dst);                  // dst[w][j] = c_j mt[w][j]
-int ensure_sweep_tables(sail_handle *h, int G);
+int ensure_sweep_tables(sail_handle *h);
+bool sweep_fits(int n_omega);                                         // tables + records within one SM's shared memory
 
 } // namespace sail

@@ -1,5 +1,5 @@
-// sweep_common.cuh — shared by the sweep-kernel translation units (sweep.cu, sweep_grp.cu): launch arguments,
-// PTX helpers, the staged proposal (row A2) and Eq. 30.  Not part of the ABI.
+// sweep_common.cuh — helpers of the sweep kernel (sweep.cu): launch arguments, PTX accessors, the DMMA warp sum,
+// the staged proposal (row A2) and Eq. 30.  Not part of the ABI.
 #pragma once
 #include "sail_internal.cuh"
 
@@ -7,8 +7,8 @@ namespace sail {
 
 struct SweepArgs {
     int n_omega, n_tau;
-    long long W, n_groups;
-    double A, B, omega_mid0, domega, eta, amp_p, amp_m, y_min;
+    long long W;
+    double A, B, domega, eta, amp_p, amp_m, y_min;
     int amp_mode;
     uint32_t seed_lo, seed_hi;
     const double *Wj, *fj, *ratio, *E0, *invd, *omega;
@@ -75,28 +75,12 @@ __device__ __forceinline__ void stg_f64_if(double *p, double v, int pred)
 {
     asm volatile("{\n\t.reg .pred q;\n\tsetp.ne.s32 q, %2, 0;\n\t@q st.global.f64 [%0], %1;\n\t}" :: "l"(p), "d"(v), "r"(pred) : "memory");
 }
-// predicated (not branched) FP64 updates: lanes of walkers that did not accept keep their state without
-// the warp diverging
-__device__ __forceinline__ void add_if(double &x, double y, int pred)
-{
-    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %2, 0;\n\t@p add.rn.f64 %0, %0, %1;\n\t}" : "+d"(x) : "d"(y), "r"(pred));
-}
-__device__ __forceinline__ void fma_if(double &x, double a, double b, int pred)
-{
-    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %3, 0;\n\t@p fma.rn.f64 %0, %1, %2, %0;\n\t}" : "+d"(x) : "d"(a), "d"(b), "r"(pred));
-}
-__device__ __forceinline__ void mul_if(double &x, double a, int pred)
-{
-    asm("{\n\t.reg .pred p;\n\tsetp.ne.s32 p, %2, 0;\n\t@p mul.rn.f64 %0, %0, %1;\n\t}" : "+d"(x) : "d"(a), "r"(pred));
-}
-
-
 
 // Sum of one double per lane over the whole warp, result in every lane, on the FP64 tensor-core path (DMMA, no
 // shuffles): D = ones(8x4) . B(4x8) with B[k = lane%4][n = lane/4] = x puts the 8 column sums in every row of D;
 // a lane owns columns 2(lane%4), 2(lane%4)+1, and their sum h(lane%4), fed through the same product, is the total.
-// Measured on B200: a DMMA m8n8k4 occupies the FP64 pipe like 8 DFMAs (it has no unit of its own), latency 27
-// cycles; the 5-stage shuffle butterfly costs 10 cycles of the SM's shared-memory/shuffle pipe and ~190 of latency.
+// Measured on B200 (sail_microbench): a DMMA m8n8k4 occupies the FP64 pipe like 8 DFMAs (it has no unit of its own);
+// the two products + DADD take ~77 cycles of latency against ~190 for the 5-stage shuffle butterfly.
 __device__ __forceinline__ double warp_sum_dmma(double x)
 {
     double c0, c1, t0, t1;
@@ -106,25 +90,7 @@ __device__ __forceinline__ double warp_sum_dmma(double x)
     const double h = c0 + c1;
     asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%4,%4};"
         : "=d"(t0), "=d"(t1) : "d"(one), "d"(h), "d"(zero));
-    return t0;
-}
-
-// The same for groups of G = 8, 16 or 32 consecutive lanes (every lane gets the sum over ITS group): after the first
-// product and the pair sum, h held by a lane with lane % 4 = q is the sum over lanes 8q .. 8q+7; the second product
-// takes A[m][k] = 1 where octet k belongs to the group of row m (m = lane / 4 is the row a lane reads back).
-template <int G>
-__device__ __forceinline__ double group_sum_dmma(double x)
-{
-    const int lane = threadIdx.x & 31;
-    const int m = lane >> 2, k = lane & 3;
-    const double sel = (G == 32) ? 1.0 : (G == 16) ? (((k < 2) == (m < 4)) ? 1.0 : 0.0) : ((k == (m >> 1)) ? 1.0 : 0.0);
-    double c0, c1, t0, t1;
-    const double one = 1.0, zero = 0.0;
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%4,%4};"
-        : "=d"(c0), "=d"(c1) : "d"(one), "d"(x), "d"(zero));
-    const double h = c0 + c1;
-    asm("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%4,%4};"
-        : "=d"(t0), "=d"(t1) : "d"(sel), "d"(h), "d"(zero));
+    (void)t1;
     return t0;
 }
 
@@ -139,38 +105,31 @@ __device__ __forceinline__ double amp_factor(const SweepArgs &P, int acc_sweep, 
     return yy < P.y_min ? P.y_min : yy;
 }
 
-constexpr int kRecMaskBytes = 80;
-// record: [0] p, s (int32), alpha = rho - 1   [16] delta_p, delta_s   [32] delta_p r_p, delta_s r_s
-//         [48] r_p + r_s, -(r_p r_s)          [64] thr = -T ln u_acc, 1/rho
-struct MoveRegs { int p, s; double alpha, dp, ds; };   // the part of a proposal its own lane keeps for the positivity screen
-__device__ __forceinline__ MoveRegs propose_mask(const SweepArgs &P, uint32_t walker, uint32_t sweep, uint32_t move, double y, double T,
-                                             const double *s_ratio, const double *s_invd, const double *s_wm, unsigned char *rec)
+__device__ __forceinline__ double u01(uint32_t x) { return ((double)x + 0.5) * 2.3283064365386962890625e-10; }
+
+// One staged proposal in shared memory (80 bytes; 112 with the index walk):
+//   [ 0] p, s (int32), alpha = rho - 1   [16] delta_p, delta_s (Eq. 20-21)   [32] delta_p r_p, delta_s r_s
+//   [48] r_p + r_s, -(r_p r_s)           [64] thr = -T ln u_acc, 1/rho
+//   [80] [96] (walk only) the Philox words of the first two walk steps
+constexpr int kRecBytes = 80;
+constexpr int kRecWalkBytes = 112;
+
+// the index-dependent half of a proposal: Eq. 20-21 in the method's operation order (only the division by
+// (p - s) domega is a multiplication by the correctly rounded reciprocal: delta within 2 ulp of the division form) and
+// the coefficients of the two-term recurrence of delta_p E_p + delta_s E_s along a lane's tau-points
+__device__ __forceinline__ void write_indexed(const SweepArgs &P, int p, int s, double alpha, const double *s_ratio,
+                                              const double *s_invd, double wm_s, double wm_p, unsigned char *rec)
 {
-    uint32_t x[4];
-    philox4x32_10(walker, sweep, move, 0u, P.seed_lo, P.seed_hi, x);
-    const int p = (int)__umulhi(x[0], (uint32_t)P.n_omega);
-    int s = (int)__umulhi(x[1], (uint32_t)(P.n_omega - 1));
-    s += (s >= p) ? 1 : 0;
-    const double u_rho = ((double)x[2] + 0.5) * 2.3283064365386962890625e-10;
-    const double u_acc = ((double)x[3] + 0.5) * 2.3283064365386962890625e-10;
-    const double rho = __dsub_rn(1.0, __dmul_rn(__dmul_rn(y, P.eta), __dsub_rn(__dmul_rn(2.0, u_rho), 1.0)));
-    const double alpha = __dsub_rn(rho, 1.0);
-    const double omr = __dsub_rn(1.0, rho);
+    const double omr = -alpha;                           // 1 - rho, exact like alpha = rho - 1
     const int dps = p - s;
     const double inv = (dps > 0) ? s_invd[dps] : -s_invd[-dps];
-    const double dp = __dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[s]))), inv);
-    const double ds = -__dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, s_wm[p]))), inv);
-    const double thr = -T * log(u_acc);
+    const double dp = __dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, wm_s))), inv);
+    const double ds = -__dmul_rn(__dmul_rn(omr, __dsub_rn(P.B, __dmul_rn(P.A, wm_p))), inv);
     const double rp = s_ratio[p], rs = s_ratio[s];
     *reinterpret_cast<int4 *>(rec) = make_int4(p, s, __double2loint(alpha), __double2hiint(alpha));
     *reinterpret_cast<double2 *>(rec + 16) = make_double2(dp, ds);
     *reinterpret_cast<double2 *>(rec + 32) = make_double2(dp * rp, ds * rs);
     *reinterpret_cast<double2 *>(rec + 48) = make_double2(rp + rs, -(rp * rs));
-    *reinterpret_cast<double2 *>(rec + 64) = make_double2(thr, fast_recip(rho));
-    return MoveRegs{p, s, alpha, dp, ds};
 }
-
-// implemented in sweep_grp.cu: the grouped screened kernel (G = 8, 16 or 32 lanes per walker)
-int launch_sweep_grp(sail_handle *h, SweepArgs &args, int G, int C, bool trace, int flavour);
 
 } // namespace sail
