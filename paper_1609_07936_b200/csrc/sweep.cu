@@ -69,7 +69,7 @@ __device__ __forceinline__ void index_walk(const SweepArgs &P, uint32_t walker, 
         uint32_t xw[4];
         words(l, xw);
         const int c = (int)__umulhi(xw[0], (uint32_t)P.n_omega);
-        if (__dmul_rn(u01(xw[1]), ldg_f64(a_row + p)) < ldg_f64(a_row + c)) p = c;
+        if (__dmul_rn(u01(xw[1]), ld_f64(a_row + p)) < ld_f64(a_row + c)) p = c;
     }
     s = s_raw + (s_raw >= p ? 1 : 0);
     for (int l = 0; l < wl; ++l) {
@@ -77,7 +77,7 @@ __device__ __forceinline__ void index_walk(const SweepArgs &P, uint32_t walker, 
         words(l, xw);
         int c = (int)__umulhi(xw[2], (uint32_t)(P.n_omega - 1));
         c += (c >= p) ? 1 : 0;
-        if (__dmul_rn(u01(xw[3]), ldg_f64(a_row + s)) < ldg_f64(a_row + c)) s = c;
+        if (__dmul_rn(u01(xw[3]), ld_f64(a_row + s)) < ld_f64(a_row + c)) s = c;
     }
 }
 
@@ -100,6 +100,12 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
     for (int i = threadIdx.x; i < (int)(blockDim.x * (kRec / 4)); i += blockDim.x)
         reinterpret_cast<uint32_t *>(s_recs)[i] = 0u;
     __syncthreads();
+    // WALK: the walk gathers the spectrum at random bins right after an accepted move has stored two of them; from
+    // global memory every such gather waits for L2 (the stores drop the lines from L1), so each warp keeps a copy of its
+    // walker's spectrum in shared memory when the copies of all resident warps fit
+    double *s_spec = nullptr;
+    if (WALK && P.spec_smem)
+        s_spec = reinterpret_cast<double *>(s_recs + (size_t)(blockDim.x >> 5) * 32 * kRec) + (size_t)(threadIdx.x >> 5) * n_omega_pad;
 
     const int lane = threadIdx.x & 31;
     const int warp = threadIdx.x >> 5;
@@ -131,6 +137,12 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
             Wt[i] = ok ? P.Wj[j] : 0.0;
             if (W2REG) W2[i] = Wt[i] + Wt[i];
             d[i] = 0.0;
+        }
+        const double *walk_src = a_all + wbase;           // where the index walk and (WALK) the screen read the spectrum
+        if (WALK && s_spec) {
+            for (int k = lane; k < n_omega; k += G) s_spec[k] = a_all[(size_t)wbase + k];
+            walk_src = s_spec;
+            __syncwarp();
         }
         double chi2 = P.chi2[w];
         double g = 1.0, ginv = 1.0;
@@ -169,7 +181,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                             if (l < wl) philox4x32_10((uint32_t)w, sweep_abs, (uint32_t)(m0 + lane), (uint32_t)(2 + l), P.seed_lo, P.seed_hi, xw);
                             *reinterpret_cast<uint4 *>(my_rec_w + 80 + 16 * l) = make_uint4(xw[0], xw[1], xw[2], xw[3]);
                         }
-                        index_walk(P, (uint32_t)w, sweep_abs, (uint32_t)(m0 + lane), wl, my_rec_w, a_all + wbase, p, dr.s_raw, s);
+                        index_walk(P, (uint32_t)w, sweep_abs, (uint32_t)(m0 + lane), wl, my_rec_w, walk_src, p, dr.s_raw, s);
                     }
                     write_indexed(P, p, s, dr.alpha, s_ratio, s_invd, wm(s), wm(p), my_rec_w);
                 }
@@ -187,8 +199,8 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                 auto screen = [&](uint32_t sel) -> uint32_t {
                     const int4 q0 = lds_s32x4(rec_own);
                     const double2 qd = lds_f64x2(rec_own + 16);
-                    const double a_p = ACACHE ? ca_p : ldg_f64(elem_ptr(a_all, wbase + (uint32_t)q0.x));
-                    const double a_s = ACACHE ? ca_s : ldg_f64(elem_ptr(a_all, wbase + (uint32_t)q0.y));
+                    const double a_p = ACACHE ? ca_p : WALK ? ld_f64(walk_src + q0.x) : ldg_f64(elem_ptr(a_all, wbase + (uint32_t)q0.x));
+                    const double a_s = ACACHE ? ca_s : WALK ? ld_f64(walk_src + q0.y) : ldg_f64(elem_ptr(a_all, wbase + (uint32_t)q0.y));
                     const double qa = __hiloint2double(q0.w, q0.z);
                     const double gn = fma(qa, g, g);
                     const double x_p = fma(gn, a_p, qd.x);
@@ -251,6 +263,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                         const double newp = apn * ginv, news = asn * ginv;
                         stg_f64_if(elem_ptr(a_all, wbase + (uint32_t)r0.x), newp, mine);
                         stg_f64_if(elem_ptr(a_all, wbase + (uint32_t)r0.y), news, mine);
+                        if (WALK && s_spec && mine) { s_spec[r0.x] = newp; s_spec[r0.y] = news; }
                         acc_sweep++;
                         if (TRACE) tr_acc |= 1u << m;
                         const uint32_t behind = valid & ~((2u << m) - 1u);
@@ -270,7 +283,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                             if (((behind >> lane) & 1u) && wl > 0) {
                                 const int2 q = *reinterpret_cast<const int2 *>(my_rec_w);
                                 int p = dr.p, s = q.y;
-                                index_walk(P, (uint32_t)w, sweep_abs, (uint32_t)(m0 + lane), wl, my_rec_w, a_all + wbase, p, dr.s_raw, s);
+                                index_walk(P, (uint32_t)w, sweep_abs, (uint32_t)(m0 + lane), wl, my_rec_w, walk_src, p, dr.s_raw, s);
                                 if (p != q.x || s != q.y) write_indexed(P, p, s, dr.alpha, s_ratio, s_invd, wm(s), wm(p), my_rec_w);
                             }
                             __syncwarp();
@@ -302,7 +315,11 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                 __syncwarp();
             }
             // ---- end of sweep: fold the lazy scale (Eq. 19), counters, y (row A6, Eq. 30) ----------------
-            for (int k = lane; k < n_omega; k += G) a_all[(size_t)wbase + k] *= g;
+            for (int k = lane; k < n_omega; k += G) {
+                const double v = ((WALK && s_spec) ? s_spec[k] : a_all[(size_t)wbase + k]) * g;
+                a_all[(size_t)wbase + k] = v;
+                if (WALK && s_spec) s_spec[k] = v;
+            }
             g = 1.0;
             ginv = 1.0;
             if (lane == 0) {
@@ -408,9 +425,12 @@ static int launch_variant(sail_handle *h, SweepArgs &args)
     if (warps < 1) warps = 1;
     // large omega grids: fewer warps per CTA until tables + records fit the 227 KB of one SM
     while (warps > 1 && sweep_smem_bytes(args.n_omega, warps, WALK) > 227 * 1024) --warps;
-    const size_t smem = sweep_smem_bytes(args.n_omega, warps, WALK);
+    size_t smem = sweep_smem_bytes(args.n_omega, warps, WALK);
     if (smem > 227 * 1024)
         return set_err(h, SAIL_ERR_ARG, "sweep tables need %zu bytes of shared memory (> 227 KB)", smem);
+    const size_t spec_bytes = (size_t)warps * ((args.n_omega + 1) & ~1) * sizeof(double);
+    args.spec_smem = (WALK && smem + spec_bytes <= 227 * 1024) ? 1 : 0;
+    if (args.spec_smem) smem += spec_bytes;
     long long ctas = (args.W + warps - 1) / warps;
     if (ctas > h->num_sms) ctas = h->num_sms;
     void (*kern)(const SweepArgs) = sweep_kernel<C, MAXW, FACT, TRACE, W2REG, ACACHE, WALK>;
@@ -424,8 +444,11 @@ template <int C, int MAXW, bool W2REG, bool ACACHE>
 static int launch_c(sail_handle *h, SweepArgs &a, bool trace)
 {
     const bool walk = a.walk_len > 0;
+    // the walk reads the spectrum at random bins: fewer warps per SM (24 at C <= 4) keep records + tables within the
+    // 164 KB shared-memory carve-out, which leaves the L1 large enough for the spectra of the resident walkers
+    constexpr int MAXW_WALK = MAXW;
 #define SAIL_PICK(FA, TR)                                                                    \
-    return walk ? launch_variant<C, MAXW, FA, TR, W2REG, false, true>(h, a)                 \
+    return walk ? launch_variant<C, MAXW_WALK, FA, TR, W2REG, false, true>(h, a)            \
                 : launch_variant<C, MAXW, FA, TR, W2REG, ACACHE, false>(h, a);
     if (a.fact) { if (trace) { SAIL_PICK(true, true) } else { SAIL_PICK(true, false) } }
     if (trace) { SAIL_PICK(false, true) }

@@ -19,6 +19,7 @@ struct SweepArgs {
     long long sweep0;
     int n_sweeps;
     int walk_len;                      // length of the index-selection walk (section 2.3); 0 = uniform indices
+    int spec_smem;                     // WALK: every warp keeps a copy of its walker's spectrum in shared memory
     double walk_uniform;               // fraction of moves that keep the uniform indices (:158)
     long long trace_lo, trace_hi;
     sail_trace_rec *trace;
@@ -68,6 +69,13 @@ __device__ __forceinline__ double ldg_f64(const double *p)
 {
     double v;
     asm volatile("ld.global.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
+    return v;
+}
+// generic-address load (shared or global), never cached in a register across a warp synchronisation
+__device__ __forceinline__ double ld_f64(const double *p)
+{
+    double v;
+    asm volatile("ld.f64 %0, [%1];" : "=d"(v) : "l"(p) : "memory");
     return v;
 }
 // predicated (not branched) store: only the lanes with pred != 0 write
