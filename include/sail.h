@@ -159,11 +159,12 @@ SAIL_API int sail_branch(sail_t *h, double T, double t_imprint, sail_branch_info
 /*
  * sail_branch_fraction — the paper's own way of fixing the branching strength (:174, :220): "Delta is found
  * numerically such that a given fraction of walkers is assigned a zero multiplier" (the paper branches a quarter of
- * the walkers).  The inverse temperature Delta = 1/T of sail_branch is searched (bracketing from 1/(chi2_max -
- * chi2_min), then 40 bisection steps; every trial runs the multiplier chain on the device with the same comb
- * offset, reading B6) for the smallest value that gives at least floor(fraction W + 1/2) zeros; then the
- * event runs at that temperature.  *T_found (HOST, may be NULL) receives it; 0 means no event happened (all residues
- * equal, or fraction W rounds to 0).  Other arguments as sail_branch.  Synchronises the stream (once per trial).
+ * the walkers).  The inverse temperature Delta = 1/T of sail_branch is searched on the device, inside the kernel that
+ * builds the multiplier plan (bracketing from 1/(chi2_max - chi2_min), then 40 bisection steps; every trial is one pass
+ * of the multiplier chain with the same comb offset, reading B6), for the smallest value that gives at least
+ * floor(fraction W + 1/2) zeros; then the event runs at that temperature: two kernel launches in all.  *T_found (HOST,
+ * may be NULL) receives it; 0 means no event happened (all residues equal, or fraction W rounds to 0).  Other arguments
+ * as sail_branch.  Synchronises the stream only when an output is requested.
  */
 SAIL_API int sail_branch_fraction(sail_t *h, double fraction, double t_imprint, double *T_found, sail_branch_info *info,
                                   int32_t *mult_out, int64_t *donor_out);
@@ -201,7 +202,7 @@ typedef struct {
     double  branch_fraction;    /* > 0: branch that fraction of the walkers (sail_branch_fraction; paper: 1/4, :220);
                                  * 0: branch at the block's own 1/T (sail_branch)                                   */
     const double *T_override;   /* HOST [n_blocks] or NULL: use these temperatures instead of the rule (tests)      */
-    sail_anneal_params anneal;  /* eta, Eq. 30 parameters, kernel form, traces for the sweeps of the blocks         */
+    sail_anneal_params anneal;  /* eta, Eq. 30 parameters, resync period, index walk; trace and flags must be NULL       */
 } sail_selfcool_params;
 
 /*
@@ -209,7 +210,9 @@ typedef struct {
  * section 2.4 (:160-162): before each block the residues chi2_ave, chi2_min are measured (sail_chi2_stats), the block's
  * temperature follows from them (block 0: T_start starting residues; boil: chi2_ave; ramp: linear to chi2_min; freeze-out:
  * below chi2_min, ~ 1 / blocks), then sweeps_per_block sweeps at that temperature, sail_smooth (if smooth_s > 0) and
- * one sail_branch at 1/T.  T_out, chi2_ave_out, chi2_min_out: HOST [n_blocks] or NULL.  Synchronises once per block.
+ * one sail_branch at 1/T.  The feedback loop runs on the device (statistics, rule, schedule slice, branching parameters):
+ * no host synchronisation inside a block.  T_out, chi2_ave_out, chi2_min_out: HOST [n_blocks] or NULL, copied once at
+ * the end (once per 4096 blocks).  Errors: SAIL_ERR_ARG also when the rule reaches T <= 0 (reported at the end).
  */
 SAIL_API int sail_anneal_selfcool(sail_t *h, const sail_selfcool_params *p, int64_t n_blocks, double *T_out,
                                   double *chi2_ave_out, double *chi2_min_out);

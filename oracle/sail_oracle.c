@@ -539,7 +539,15 @@ void orc_smooth(const orc_problem *P, int64_t W, double s, double *a, double *M,
         for (int k = 0; k < n; ++k) { A1 += tmp[k]; B1 += tmp[k] * (P->omega[k] + half); }
         const double wbar = B1 / A1;
         for (int k = 0; k < n; ++k) { const double dw = (P->omega[k] + half) - wbar; V += tmp[k] * dw * dw; }
-        const double kappa = (V > 0.0) ? (P->B - B1) / V : 0.0;
+        double kappa = (V > 0.0) ? (P->B - B1) / V : 0.0;
+        /* reading S2, positivity (Eq. 10 needs a_k >= 0): the tilt factor 1 + kappa (w^m_k - wbar) is linear in k, so it
+         * is smallest at one of the two end bins; kappa is clamped so that it stays >= 0 there (the second sum rule is
+         * then restored only in part; s of a few percent never gets near the clamp) */
+        {
+            const double d_lo = (P->omega[0] + half) - wbar, d_hi = (P->omega[n - 1] + half) - wbar;
+            if (1.0 + kappa * d_lo < 0.0) kappa = -1.0 / d_lo;
+            if (1.0 + kappa * d_hi < 0.0) kappa = -1.0 / d_hi;
+        }
         for (int k = 0; k < n; ++k) row[k] = tmp[k] * (1.0 + kappa * ((P->omega[k] + half) - wbar));
         free(tmp);
         orc_forward(n, P->n_tau, P->K, row, M + (size_t)w * P->n_tau);

@@ -2,14 +2,13 @@
 // DESIGN.md §2): fixed-point weights -> integer prefix sum -> comb multipliers (sum m = W exactly) ->
 // donor map by binary search -> coalesced 128-bit imprint copy of (spectrum, model) + residue.
 #include "sail_internal.cuh"
+#include <cooperative_groups.h>
 #include <math.h>
 #include <string.h>
 
 namespace sail {
 
-constexpr int kScanThreads = 256;
-constexpr int kScanItems = 4;
-constexpr int kScanTile = kScanThreads * kScanItems;   // 1024 elements per CTA
+namespace cg = cooperative_groups;
 
 // Order-preserving key of a double: the running residue chi2_0 + sum dchi2 can dip below zero near an exact fit, so
 // the plain bit pattern (valid for values >= 0 only) is not enough.  Negative values have all bits flipped, the others
@@ -24,150 +23,231 @@ __device__ __forceinline__ double key_value(unsigned long long k)
     return __longlong_as_double((long long)((k >> 63) ? (k & 0x7fffffffffffffffull) : ~k));
 }
 
-__global__ void chi2_min_kernel(long long W, const double *__restrict__ chi2, unsigned long long *scalars)
-{
-    unsigned long long m = ~0ull;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
-        const unsigned long long b = ordered_key(chi2[i]);
-        m = b < m ? b : m;
-    }
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-        const unsigned long long o = __shfl_xor_sync(0xffffffffu, m, off);
-        m = o < m ? o : m;
-    }
-    if ((threadIdx.x & 31) == 0) atomicMin(scalars + 0, m);
-}
+// ---- the whole multiplier plan of one branching event in ONE cooperative kernel -----------------------------------
+// weights (B1, B3) -> u64 inclusive scan -> comb multipliers (B2) -> scans of recipient flags and donor extras -> donor
+// map (B4), with grid-wide barriers between the phases instead of kernel boundaries; in the search modes the first two
+// phases run once per trial of 1/T (reading B6: bracketing by doubling / halving from 1/(chi2_max - chi2_min), then 40
+// bisection steps; fp64 arithmetic steered by integer counts, identical on every CTA, so the grid stays in step).
+// Every CTA owns a contiguous chunk of walkers; all integer arithmetic is order independent, so the multipliers are the
+// ones of the definition bit for bit.
+constexpr int kPlanThreads = 512;
+constexpr int kPlanWarps = kPlanThreads / 32;
 
-// B1 + B3: e_i = exp(-(chi2_i - chi2_min)/T), E_i = floor(e_i 2^40)
-__global__ void weights_kernel(long long W, const double *__restrict__ chi2, double T,
-                               const unsigned long long *scalars, unsigned long long *ehat)
-{
-    const double cmin = key_value(scalars[0]);
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
-        // chi2_i >= chi2_min makes the exponent <= 0 and the weight <= 2^40; a NaN residue gets weight 0
-        const double e = exp(-(chi2[i] - cmin) / T);
-        ehat[i] = (e == e) ? (unsigned long long)floor(fmin(e, 1.0) * 1099511627776.0) : 0ull;
-    }
-}
+struct PlanArgs {
+    long long W;
+    const double *chi2;
+    int mode;                          // 0: T given; 1: search for `fraction`; 2 / 3: the same with T / fraction from ctl[0] / ctl[1]
+    double T, fraction;
+    const double *ctl;                 // DEVICE (T, fraction) of modes 2, 3
+    uint32_t seed_lo, seed_hi, sweep;
+    unsigned long long *ehat, *scanA, *scanB, *part, *scalars;
+    int32_t *mult;
+    int64_t *donor_of, *rec_list;
+};
 
-// ---- three-phase inclusive scan of u64 arrays (blockIdx.y selects the array) -----------------------
-struct ScanArrays { unsigned long long *arr[2]; unsigned long long *sums[2]; };
-
-__global__ void __launch_bounds__(kScanThreads) scan_tiles_kernel(long long n, ScanArrays S)
+__device__ __forceinline__ unsigned long long warp_incl_scan(unsigned long long v, int lane)
 {
-    __shared__ unsigned long long warp_tot[kScanThreads / 32];
-    unsigned long long *x = S.arr[blockIdx.y];
-    const long long base = (long long)blockIdx.x * kScanTile + (long long)threadIdx.x * kScanItems;
-    unsigned long long v[kScanItems], run = 0;
-#pragma unroll
-    for (int i = 0; i < kScanItems; ++i) {
-        v[i] = (base + i < n) ? x[base + i] : 0ull;
-        run += v[i];
-        v[i] = run;
-    }
-    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
-    unsigned long long inc = run;
 #pragma unroll
     for (int off = 1; off < 32; off <<= 1) {
-        const unsigned long long o = __shfl_up_sync(0xffffffffu, inc, off);
-        if (lane >= off) inc += o;
+        const unsigned long long o = __shfl_up_sync(0xffffffffu, v, off);
+        if (lane >= off) v += o;
     }
-    if (lane == 31) warp_tot[wid] = inc;
+    return v;
+}
+// inclusive scan of one value per thread over the CTA; *total = sum over the CTA (sm: kPlanWarps slots, reusable after return)
+__device__ __forceinline__ unsigned long long block_incl_scan(unsigned long long v, unsigned long long *sm, unsigned long long *total)
+{
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+    const unsigned long long inc = warp_incl_scan(v, lane);
+    if (lane == 31) sm[wid] = inc;
     __syncthreads();
-    unsigned long long prefix = inc - run;
-    for (int w2 = 0; w2 < wid; ++w2) prefix += warp_tot[w2];
+    unsigned long long prefix = 0, tot = 0;
 #pragma unroll
-    for (int i = 0; i < kScanItems; ++i)
-        if (base + i < n) x[base + i] = v[i] + prefix;
-    if (threadIdx.x == kScanThreads - 1) S.sums[blockIdx.y][blockIdx.x] = prefix + run;
+    for (int w2 = 0; w2 < kPlanWarps; ++w2) { const unsigned long long t = sm[w2]; if (w2 < wid) prefix += t; tot += t; }
+    __syncthreads();
+    *total = tot;
+    return inc + prefix;
 }
-
-__global__ void scan_sums_kernel(int n_tiles, ScanArrays S)
+template <int OP>   // 0 sum, 1 min, 2 max
+__device__ __forceinline__ unsigned long long block_reduce(unsigned long long v, unsigned long long *sm)
 {
-    // few tiles (W/1024): one thread per array is enough and keeps the result exact and ordered
-    if (threadIdx.x == 0) {
-        unsigned long long *s = S.sums[blockIdx.x];
-        unsigned long long run = 0;
-        for (int i = 0; i < n_tiles; ++i) { const unsigned long long t = s[i]; s[i] = run; run += t; }
-    }
-}
-
-__global__ void __launch_bounds__(kScanThreads) scan_add_kernel(long long n, ScanArrays S)
-{
-    unsigned long long *x = S.arr[blockIdx.y];
-    const unsigned long long off = S.sums[blockIdx.y][blockIdx.x];
-    const long long base = (long long)blockIdx.x * kScanTile + (long long)threadIdx.x * kScanItems;
-#pragma unroll
-    for (int i = 0; i < kScanItems; ++i)
-        if (base + i < n) x[base + i] += off;
-}
-
-static int scan_inclusive(sail_handle *h, long long n, int n_arrays, unsigned long long *a0, unsigned long long *a1)
-{
-    const int tiles = (int)((n + kScanTile - 1) / kScanTile);
-    ScanArrays S;
-    S.arr[0] = a0; S.arr[1] = a1;
-    S.sums[0] = h->br.block_sums; S.sums[1] = h->br.block_sums + tiles;
-    scan_tiles_kernel<<<dim3(tiles, n_arrays), kScanThreads, 0, h->stream>>>(n, S);
-    SAIL_LAUNCH_OK(h, "scan_tiles_kernel");
-    if (tiles > 1) {
-        scan_sums_kernel<<<n_arrays, 32, 0, h->stream>>>(tiles, S);
-        SAIL_LAUNCH_OK(h, "scan_sums_kernel");
-        scan_add_kernel<<<dim3(tiles, n_arrays), kScanThreads, 0, h->stream>>>(n, S);
-        SAIL_LAUNCH_OK(h, "scan_add_kernel");
-    }
-    return SAIL_OK;
-}
-
-// B2: comb multipliers m_i = floor((C_i W + Xi)/S) - floor((C_{i-1} W + Xi)/S), Xi = (x0 S) >> 32
-__global__ void multipliers_kernel(long long W, const unsigned long long *__restrict__ Cinc, uint32_t seed_lo,
-                                   uint32_t seed_hi, uint32_t sweep, int32_t *mult, unsigned long long *is_rec,
-                                   unsigned long long *extras, unsigned long long *scalars)
-{
-    const unsigned long long S = Cinc[W - 1];
-    uint32_t x[4];
-    philox4x32_10(0u, sweep, 0u, 1u, seed_lo, seed_hi, x);
-    const unsigned __int128 Xi = ((unsigned __int128)x[0] * S) >> 32;
-    int mmax = 0;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
-        const unsigned long long cprev = i ? Cinc[i - 1] : 0ull;
-        const unsigned long long hi = (unsigned long long)(((unsigned __int128)Cinc[i] * (unsigned long long)W + Xi) / S);
-        const unsigned long long lo = (unsigned long long)(((unsigned __int128)cprev * (unsigned long long)W + Xi) / S);
-        const int m = (int)(hi - lo);
-        mult[i] = m;
-        is_rec[i] = (m == 0) ? 1ull : 0ull;
-        extras[i] = (m > 1) ? (unsigned long long)(m - 1) : 0ull;
-        mmax = m > mmax ? m : mmax;
-    }
 #pragma unroll
     for (int off = 16; off > 0; off >>= 1) {
-        const int o = __shfl_xor_sync(0xffffffffu, mmax, off);
-        mmax = o > mmax ? o : mmax;
+        const unsigned long long o = __shfl_xor_sync(0xffffffffu, v, off);
+        v = (OP == 0) ? v + o : (OP == 1) ? (o < v ? o : v) : (o > v ? o : v);
     }
-    if ((threadIdx.x & 31) == 0) atomicMax(scalars + 3, (unsigned long long)mmax);
-    if (blockIdx.x == 0 && threadIdx.x == 0) scalars[1] = S;
+    if ((threadIdx.x & 31) == 0) sm[threadIdx.x >> 5] = v;
+    __syncthreads();
+    unsigned long long r = sm[0];
+#pragma unroll
+    for (int w2 = 1; w2 < kPlanWarps; ++w2) { const unsigned long long o = sm[w2]; r = (OP == 0) ? r + o : (OP == 1) ? (o < r ? o : r) : (o > r ? o : r); }
+    __syncthreads();
+    return r;
+}
+// (sum of part[0..n), sum of part[0..me)) — every thread gets both
+__device__ __forceinline__ void grid_totals(const unsigned long long *part, int n, int me, unsigned long long *sm,
+                                            unsigned long long *total, unsigned long long *before)
+{
+    unsigned long long t = 0, b = 0;
+    for (int c = threadIdx.x; c < n; c += blockDim.x) { const unsigned long long v = part[c]; t += v; if (c < me) b += v; }
+    *total = block_reduce<0>(t, sm);
+    *before = block_reduce<0>(b, sm);
 }
 
-// B4: recipient of rank r takes the donor with X_i <= r < X_i + x_i (binary search on the inclusive scan)
-__global__ void donor_map_kernel(long long W, const int32_t *__restrict__ mult, const unsigned long long *__restrict__ rec_inc,
-                                 const unsigned long long *__restrict__ ext_inc, int64_t *donor_of, int64_t *rec_list,
-                                 unsigned long long *scalars)
+__global__ void __launch_bounds__(kPlanThreads) branch_plan_kernel(const PlanArgs a)
 {
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
+    cg::grid_group grid = cg::this_grid();
+    __shared__ unsigned long long sm[kPlanWarps];
+    __shared__ unsigned long long sm_hi[kPlanThreads + 1];
+    const int G = gridDim.x, me = blockIdx.x, tid = threadIdx.x;
+    const long long W = a.W;
+    const long long chunk = (W + G - 1) / G;
+    const long long c0 = (long long)me * chunk < W ? (long long)me * chunk : W;
+    const long long c1 = c0 + chunk < W ? c0 + chunk : W;
+    unsigned long long *pE = a.part, *pZ = a.part + G, *pX = a.part + 2 * G, *pMin = a.part + 3 * G, *pMax = a.part + 4 * G, *pM = a.part + 5 * G;
+
+    // ---- smallest / largest residue --------------------------------------------------------------------
+    unsigned long long kmin = ~0ull, kmax = 0ull;
+    for (long long i = c0 + tid; i < c1; i += kPlanThreads) {
+        const unsigned long long k = ordered_key(a.chi2[i]);
+        kmin = k < kmin ? k : kmin;
+        kmax = k > kmax ? k : kmax;
+    }
+    kmin = block_reduce<1>(kmin, sm);
+    kmax = block_reduce<2>(kmax, sm);
+    if (tid == 0) { pMin[me] = kmin; pMax[me] = kmax; }
+    grid.sync();
+    kmin = ~0ull; kmax = 0ull;
+    for (int c = tid; c < G; c += kPlanThreads) { kmin = pMin[c] < kmin ? pMin[c] : kmin; kmax = pMax[c] > kmax ? pMax[c] : kmax; }
+    kmin = block_reduce<1>(kmin, sm);
+    kmax = block_reduce<2>(kmax, sm);
+    const double cmin = key_value(kmin), cmax = key_value(kmax);
+
+    uint32_t x[4];
+    philox4x32_10(0u, a.sweep, 0u, 1u, a.seed_lo, a.seed_hi, x);
+
+    // one pass of the multiplier chain at temperature T; final: also multipliers, recipient / extras scans.
+    // Returns the number of zero multipliers over the whole population.
+    auto pass = [&](double T, bool final) -> unsigned long long {
+        // B1 + B3: e_i = exp(-(chi2_i - chi2_min)/T), E_i = floor(e_i 2^40); inclusive scan within the chunk
+        unsigned long long carry = 0;
+        for (long long t0 = c0; t0 < c1; t0 += kPlanThreads) {
+            const long long i = t0 + tid;
+            unsigned long long E = 0;
+            if (i < c1) {
+                // chi2_i >= chi2_min makes the exponent <= 0 and the weight <= 2^40; a NaN residue gets weight 0
+                const double e = exp(-(a.chi2[i] - cmin) / T);
+                E = (e == e) ? (unsigned long long)floor(fmin(e, 1.0) * 1099511627776.0) : 0ull;
+            }
+            unsigned long long tot;
+            const unsigned long long inc = block_incl_scan(E, sm, &tot);
+            if (i < c1) a.ehat[i] = inc + carry;
+            carry += tot;
+        }
+        if (tid == 0) pE[me] = carry;
+        grid.sync();
+        unsigned long long S, off;
+        grid_totals(pE, G, me, sm, &S, &off);
+        // B2: comb multipliers m_i = floor((C_i W + Xi)/S) - floor((C_{i-1} W + Xi)/S), Xi = (x0 S) >> 32
+        const unsigned __int128 Xi = ((unsigned __int128)x[0] * S) >> 32;
+        auto comb = [&](unsigned long long C) { return (unsigned long long)(((unsigned __int128)C * (unsigned long long)W + Xi) / S); };
+        unsigned long long prev_hi = comb(off);          // C_{c0-1} = the sum of the chunks before this one
+        unsigned long long zeros = 0, rec_carry = 0, ext_carry = 0;
+        int mmax = 0;
+        for (long long t0 = c0; t0 < c1; t0 += kPlanThreads) {
+            const long long i = t0 + tid;
+            const unsigned long long hi = (i < c1) ? comb(a.ehat[i] + off) : 0ull;
+            sm_hi[tid + 1] = hi;
+            if (tid == 0) sm_hi[0] = prev_hi;
+            __syncthreads();
+            const int m = (i < c1) ? (int)(hi - sm_hi[tid]) : 1;
+            const long long last = (c1 - t0 < kPlanThreads ? c1 - t0 : kPlanThreads);
+            prev_hi = sm_hi[last];
+            __syncthreads();
+            if (i < c1 && m == 0) zeros++;
+            if (final) {
+                unsigned long long tr, te;
+                const unsigned long long ri = block_incl_scan((i < c1 && m == 0) ? 1ull : 0ull, sm, &tr);
+                const unsigned long long xi = block_incl_scan((i < c1 && m > 1) ? (unsigned long long)(m - 1) : 0ull, sm, &te);
+                if (i < c1) { a.mult[i] = m; a.scanA[i] = ri + rec_carry; a.scanB[i] = xi + ext_carry; }
+                rec_carry += tr; ext_carry += te;
+                if (i < c1) mmax = m > mmax ? m : mmax;
+            }
+        }
+        zeros = block_reduce<0>(zeros, sm);
+        if (final) mmax = (int)block_reduce<2>((unsigned long long)mmax, sm);
+        if (tid == 0) { pZ[me] = zeros; if (final) { pX[me] = ext_carry; pM[me] = (unsigned long long)mmax; } }
+        if (final && me == 0 && tid == 0) a.scalars[1] = S;
+        grid.sync();
+        unsigned long long zt = 0;
+        for (int c = tid; c < G; c += kPlanThreads) zt += pZ[c];
+        return block_reduce<0>(zt, sm);
+    };
+
+    // ---- temperature: given, or searched (reading B6) ------------------------------------------------------------
+    double T = (a.mode == 2) ? a.ctl[0] : a.T;
+    bool event = true;
+    if (a.mode == 1 || a.mode == 3) {
+        const double fraction = (a.mode == 3) ? a.ctl[1] : a.fraction;
+        const long long n0 = (long long)floor(fraction * (double)W + 0.5);
+        T = 0.0;
+        event = n0 > 0 && cmax > cmin;
+        if (event) {
+            double lo, hi = 1.0 / (cmax - cmin);
+            if ((long long)pass(1.0 / hi, false) >= n0) {
+                lo = 0.5 * hi;
+                for (int it = 0; it < 200 && (long long)pass(1.0 / lo, false) >= n0; ++it) { hi = lo; lo = 0.5 * lo; }
+            } else {
+                lo = hi; hi = 2.0 * hi;
+                int it = 0;
+                for (; it < 200 && (long long)pass(1.0 / hi, false) < n0; ++it) { lo = hi; hi = 2.0 * hi; }
+                if (it == 200) event = false;                // the fraction cannot be reached
+            }
+            if (event) {
+                for (int it = 0; it < 40; ++it) {
+                    const double mid = 0.5 * (lo + hi);
+                    if ((long long)pass(1.0 / mid, false) >= n0) hi = mid; else lo = mid;
+                }
+                T = 1.0 / hi;
+            }
+        }
+    }
+    if (!event) {                                            // degenerate population or nothing asked for: no recipients
+        if (me == 0 && tid == 0) {
+            a.scalars[0] = kmin; a.scalars[1] = 0; a.scalars[2] = 0; a.scalars[3] = 1;
+            a.scalars[5] = (unsigned long long)__double_as_longlong(0.0);
+        }
+        for (long long i = c0 + tid; i < c1; i += kPlanThreads) { a.mult[i] = 1; a.donor_of[i] = -1; }
+        return;
+    }
+    const unsigned long long n_rec = pass(T, true);
+    // ---- recipient ranks and donor extras: chunk-local scans -> global (B4) ----------------------------------------
+    unsigned long long tot_r, off_r, tot_x, off_x;
+    grid_totals(pZ, G, me, sm, &tot_r, &off_r);
+    grid_totals(pX, G, me, sm, &tot_x, &off_x);
+    for (long long i = c0 + tid; i < c1; i += kPlanThreads) { a.scanA[i] += off_r; a.scanB[i] += off_x; }
+    unsigned long long mm = 0;
+    for (int c = tid; c < G; c += kPlanThreads) mm = pM[c] > mm ? pM[c] : mm;
+    mm = block_reduce<2>(mm, sm);
+    if (me == 0 && tid == 0) {
+        a.scalars[0] = kmin; a.scalars[2] = n_rec; a.scalars[3] = mm;
+        a.scalars[5] = (unsigned long long)__double_as_longlong(T);
+    }
+    grid.sync();
+    // recipient of rank r takes the donor with X_i <= r < X_i + x_i (binary search on the inclusive scan of the extras)
+    for (long long i = c0 + tid; i < c1; i += kPlanThreads) {
         long long donor = -1;
-        if (mult[i] == 0) {
-            const unsigned long long r = rec_inc[i] - 1;
+        if (a.mult[i] == 0) {
+            const unsigned long long r = a.scanA[i] - 1;
             long long lo = 0, hi = W - 1;            // first index with ext_inc > r
             while (lo < hi) {
                 const long long mid = (lo + hi) >> 1;
-                if (ext_inc[mid] > r) hi = mid; else lo = mid + 1;
+                if (a.scanB[mid] > r) hi = mid; else lo = mid + 1;
             }
             donor = lo;
-            rec_list[r] = i;
+            a.rec_list[r] = i;
         }
-        donor_of[i] = donor;
-        if (i == W - 1) scalars[2] = rec_inc[i];
+        a.donor_of[i] = donor;
     }
 }
 
@@ -178,13 +258,14 @@ __global__ void donor_map_kernel(long long W, const int32_t *__restrict__ mult, 
 // is z bit for bit, so the recipient is not read at all (two streams instead of three).  All loads of a CTA's
 // pass are issued before its first store (8 x 16 B per thread in flight).
 template <bool COPY>
-__global__ void __launch_bounds__(256) imprint_kernel(int n_omega, int n_tau, double t, const int64_t *__restrict__ rec_list,
+__global__ void __launch_bounds__(256) imprint_kernel(int n_omega, int n_tau, double t_arg, const double *t_dev, const int64_t *__restrict__ rec_list,
                                                       const int64_t *__restrict__ donor_of, const unsigned long long *scalars,
                                                       double *a, double *mt, double *chi2,
                                                       const double *__restrict__ Wj, const double *__restrict__ fj)
 {
     __shared__ double red[8];
     const long long n_rec = (long long)scalars[2];
+    const double t = t_dev ? *t_dev : t_arg;           // t on the device: the self-cooling protocol (B7)
     const double omt = 1.0 - t;
     auto mix = [&](double z, double x) { return COPY ? z : __dadd_rn(__dmul_rn(t, z), __dmul_rn(omt, x)); };
     for (long long r = blockIdx.x; r < n_rec; r += gridDim.x) {
@@ -337,32 +418,32 @@ __global__ void __launch_bounds__(128) imprint_tma_kernel(int n_omega, int n_tau
     if (threadIdx.x == 0) asm volatile("cp.async.bulk.wait_group 0;" ::: "memory");
 }
 
-// weights -> scan -> multipliers -> scans -> donor map for inverse temperature 1/T; the number of recipients (zero
-// multipliers) ends up in scalars[2].  No walker state is touched.
-static int branch_plan(sail_handle *h, double T)
+// the multiplier plan (one cooperative launch); the number of recipients ends up in scalars[2], the temperature used
+// in scalars[5].  No walker state is touched.  mode / T / fraction / ctl as in PlanArgs.
+static int branch_plan(sail_handle *h, int mode, double T, double fraction, const double *ctl)
 {
-    const long long W = h->W;
     BranchScratch &b = h->br;
-    const int blocks = (int)((W + 255) / 256 < 1184 ? (W + 255) / 256 : 1184);
-    SAIL_CUDA_OK(h, cudaMemsetAsync(b.scalars, 0, 8 * sizeof(unsigned long long), h->stream));
-    SAIL_CUDA_OK(h, cudaMemsetAsync(b.scalars, 0xFF, sizeof(unsigned long long), h->stream));
-    chi2_min_kernel<<<blocks, 256, 0, h->stream>>>(W, h->st.chi2, b.scalars);
-    SAIL_LAUNCH_OK(h, "chi2_min_kernel");
-    weights_kernel<<<blocks, 256, 0, h->stream>>>(W, h->st.chi2, T, b.scalars, b.ehat);
-    SAIL_LAUNCH_OK(h, "weights_kernel");
-    int rc = scan_inclusive(h, W, 1, b.ehat, nullptr);
-    if (rc) return rc;
-    multipliers_kernel<<<blocks, 256, 0, h->stream>>>(W, b.ehat, (uint32_t)(h->seed & 0xFFFFFFFFu), (uint32_t)(h->seed >> 32),
-                                                      (uint32_t)h->sweep, b.mult, b.scanA, b.scanB, b.scalars);
-    SAIL_LAUNCH_OK(h, "multipliers_kernel");
-    rc = scan_inclusive(h, W, 2, b.scanA, b.scanB);
-    if (rc) return rc;
-    donor_map_kernel<<<blocks, 256, 0, h->stream>>>(W, b.mult, b.scanA, b.scanB, b.donor_of, b.rec_list, b.scalars);
-    SAIL_LAUNCH_OK(h, "donor_map_kernel");
+    PlanArgs a{};
+    a.W = h->W; a.chi2 = h->st.chi2; a.mode = mode; a.T = T; a.fraction = fraction; a.ctl = ctl;
+    a.seed_lo = (uint32_t)(h->seed & 0xFFFFFFFFu); a.seed_hi = (uint32_t)(h->seed >> 32); a.sweep = (uint32_t)h->sweep;
+    a.ehat = b.ehat; a.scanA = b.scanA; a.scanB = b.scanB; a.part = b.block_sums; a.scalars = b.scalars;
+    a.mult = b.mult; a.donor_of = b.donor_of; a.rec_list = b.rec_list;
+    if (h->plan_ctas == 0) {
+        int per_sm = 0;
+        SAIL_CUDA_OK(h, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, branch_plan_kernel, kPlanThreads, 0));
+        if (per_sm < 1) return set_err(h, SAIL_ERR_CUDA, "branch_plan_kernel does not fit an SM");
+        h->plan_ctas = h->num_sms;                     // one CTA per SM: all co-resident (cooperative launch)
+    }
+    int ctas = h->plan_ctas;
+    const long long need = (h->W + kPlanThreads - 1) / kPlanThreads;
+    if (need < ctas) ctas = (int)(need < 1 ? 1 : need);
+    void *args[] = {(void *)&a};
+    SAIL_CUDA_OK(h, cudaLaunchCooperativeKernel((const void *)branch_plan_kernel, dim3(ctas), dim3(kPlanThreads), args, 0, h->stream));
+    h->launches++;
     return SAIL_OK;
 }
 
-static int branch_imprint(sail_handle *h, double t_imprint)
+static int branch_imprint(sail_handle *h, double t_imprint, const double *t_dev)
 {
     const long long W = h->W;
     BranchScratch &b = h->br;
@@ -371,7 +452,7 @@ static int branch_imprint(sail_handle *h, double t_imprint)
     // recipients: 1.05 ms against 1.31 ms with plain loads); for t < 1 the plain-load kernel is the faster one
     // (1.64 ms against 1.79 ms: the combination runs out of shared memory at 2 CTAs per SM), so it keeps that path
     const size_t row_bytes = (size_t)(h->n_omega + h->n_tau) * sizeof(double);
-    const bool copy = t_imprint == 1.0;
+    const bool copy = t_imprint == 1.0 && !t_dev;
     const int nst = copy ? 3 : 2;
     const size_t tma_smem = (copy ? 1 : 2) * row_bytes * nst;
     if ((h->n_omega & 1) == 0 && (h->n_tau & 1) == 0 && tma_smem <= 96 * 1024 && copy) {
@@ -389,11 +470,11 @@ static int branch_imprint(sail_handle *h, double t_imprint)
         SAIL_LAUNCH_OK(h, "imprint_tma_kernel");
         return SAIL_OK;
     }
-    if (t_imprint == 1.0)
-        imprint_kernel<true><<<iblocks, 256, 0, h->stream>>>(h->n_omega, h->n_tau, t_imprint, b.rec_list, b.donor_of, b.scalars,
+    if (copy)
+        imprint_kernel<true><<<iblocks, 256, 0, h->stream>>>(h->n_omega, h->n_tau, t_imprint, nullptr, b.rec_list, b.donor_of, b.scalars,
                                                              h->st.a, h->st.mt, h->st.chi2, h->tab.Wj, h->tab.fj);
     else
-        imprint_kernel<false><<<iblocks, 256, 0, h->stream>>>(h->n_omega, h->n_tau, t_imprint, b.rec_list, b.donor_of, b.scalars,
+        imprint_kernel<false><<<iblocks, 256, 0, h->stream>>>(h->n_omega, h->n_tau, t_imprint, t_dev, b.rec_list, b.donor_of, b.scalars,
                                                               h->st.a, h->st.mt, h->st.chi2, h->tab.Wj, h->tab.fj);
     SAIL_LAUNCH_OK(h, "imprint_kernel");
     return SAIL_OK;
@@ -401,75 +482,28 @@ static int branch_imprint(sail_handle *h, double t_imprint)
 
 int launch_branch(sail_handle *h, double T, double t_imprint)
 {
-    int rc = branch_plan(h, T);
+    int rc = branch_plan(h, 0, T, 0.0, nullptr);
     if (rc) return rc;
-    return branch_imprint(h, t_imprint);
-}
-
-__global__ void chi2_max_kernel(long long W, const double *__restrict__ chi2, unsigned long long *dst)
-{
-    unsigned long long m = 0ull;
-    for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < W; i += (long long)gridDim.x * blockDim.x) {
-        const unsigned long long b = ordered_key(chi2[i]);
-        m = b > m ? b : m;
-    }
-#pragma unroll
-    for (int off = 16; off > 0; off >>= 1) {
-        const unsigned long long o = __shfl_xor_sync(0xffffffffu, m, off);
-        m = o > m ? o : m;
-    }
-    if ((threadIdx.x & 31) == 0) atomicMax(dst, m);
+    return branch_imprint(h, t_imprint, nullptr);
 }
 
 // SURVEY §8f row f2 (reading B6): 1/T such that `fraction` of the walkers get multiplier zero, found
-// by bracketing (doubling / halving from 1/(chi2_max - chi2_min)) and 40 bisection steps on 1/T; every trial runs the
-// multiplier chain on the device (same comb offset) and reads back one count.  Then the event itself at that T.
-int launch_branch_fraction(sail_handle *h, double fraction, double t_imprint, double *T_found)
+// inside the plan kernel (bracketing + 40 bisection steps, every trial a pass of the multiplier chain with the same comb
+// offset), then the event itself at that T.  The temperature found stays on the device (scalars[5]).
+int launch_branch_fraction(sail_handle *h, double fraction, double t_imprint)
 {
-    const long long W = h->W;
-    BranchScratch &b = h->br;
-    *T_found = 0.0;
-    const long long n0 = (long long)floor(fraction * (double)W + 0.5);
-    const int blocks = (int)((W + 255) / 256 < 1184 ? (W + 255) / 256 : 1184);
-    SAIL_CUDA_OK(h, cudaMemsetAsync(b.scalars, 0, 8 * sizeof(unsigned long long), h->stream));
-    SAIL_CUDA_OK(h, cudaMemsetAsync(b.scalars, 0xFF, sizeof(unsigned long long), h->stream));
-    chi2_min_kernel<<<blocks, 256, 0, h->stream>>>(W, h->st.chi2, b.scalars);
-    SAIL_LAUNCH_OK(h, "chi2_min_kernel");
-    chi2_max_kernel<<<blocks, 256, 0, h->stream>>>(W, h->st.chi2, b.scalars + 6);
-    SAIL_LAUNCH_OK(h, "chi2_max_kernel");
-    unsigned long long sc[8];
-    SAIL_CUDA_OK(h, cudaMemcpyAsync(sc, b.scalars, sizeof sc, cudaMemcpyDeviceToHost, h->stream));
-    SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
-    double cmin, cmax;
-    cmin = ordered_key_value(sc[0]); cmax = ordered_key_value(sc[6]);
-    if (n0 <= 0 || !(cmax > cmin)) return SAIL_OK;     // nothing to branch
-    int rc = SAIL_OK;
-    auto zeros = [&](double beta) -> long long {
-        if (rc) return 0;
-        rc = branch_plan(h, 1.0 / beta);
-        if (rc) return 0;
-        unsigned long long z = 0;
-        if (cudaMemcpyAsync(&z, b.scalars + 2, 8, cudaMemcpyDeviceToHost, h->stream) != cudaSuccess ||
-            cudaStreamSynchronize(h->stream) != cudaSuccess) { rc = set_err(h, SAIL_ERR_CUDA, "read-back of the recipient count failed"); return 0; }
-        return (long long)z;
-    };
-    double lo, hi = 1.0 / (cmax - cmin);
-    if (zeros(hi) >= n0) {
-        lo = 0.5 * hi;
-        for (int it = 0; it < 200 && zeros(lo) >= n0; ++it) { hi = lo; lo = 0.5 * lo; }
-    } else {
-        lo = hi; hi = 2.0 * hi;
-        int it = 0;
-        for (; it < 200 && zeros(hi) < n0; ++it) { lo = hi; hi = 2.0 * hi; }
-        if (it == 200) return rc;                      // the fraction cannot be reached
-    }
-    for (int it = 0; it < 40; ++it) {
-        const double mid = 0.5 * (lo + hi);
-        if (zeros(mid) >= n0) hi = mid; else lo = mid;
-    }
+    int rc = branch_plan(h, 1, 0.0, fraction, nullptr);
     if (rc) return rc;
-    *T_found = 1.0 / hi;
-    return launch_branch(h, *T_found, t_imprint);
+    return branch_imprint(h, t_imprint, nullptr);
+}
+
+// the same two events with their parameters on the device: ctl = (T, fraction, t_imprint) written by an earlier kernel
+// on the stream (the self-cooling protocol: no host round trip inside a block)
+int launch_branch_ctl(sail_handle *h, bool by_fraction, const double *ctl)
+{
+    int rc = branch_plan(h, by_fraction ? 3 : 2, 0.0, 0.0, ctl);
+    if (rc) return rc;
+    return branch_imprint(h, 0.5, ctl + 2);
 }
 
 } // namespace sail

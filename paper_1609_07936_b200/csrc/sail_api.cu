@@ -29,10 +29,11 @@ int set_err(sail_handle *h, int code, const char *fmt, ...)
 struct Layout {
     size_t off_omega, off_tau, off_c, off_Wj, off_fj, off_F, off_sigma, off_E, off_ET, off_ratio, off_invd, off_E0, off_T;
     size_t off_a, off_mt, off_chi2, off_y, off_nacc, off_neval, off_model;
-    size_t off_ehat, off_scanA, off_scanB, off_bsums, off_mult, off_donor, off_reclist, off_scalars;
+    size_t off_ehat, off_scanA, off_scanB, off_bsums, off_mult, off_donor, off_reclist, off_scalars, off_ctl, off_blockout;
     size_t total;
 };
 constexpr size_t kE0Doubles = 16384;
+constexpr size_t kSelfcoolBlocks = sail::kSelfcoolBlocksMax;
 constexpr size_t kScheduleDoubles = 32768;   // temperature schedule slice (longer schedules are uploaded in pieces)
 
 static Layout make_layout(int n_omega, int n_tau, int64_t Wmax)
@@ -52,11 +53,13 @@ static Layout make_layout(int n_omega, int n_tau, int64_t Wmax)
     L.off_nacc = take(W * u);         L.off_neval = take(W * u);
     L.off_model = take(W * n_tau * d);
     L.off_ehat = take(W * u);         L.off_scanA = take(W * u);     L.off_scanB = take(W * u);
-    L.off_bsums = take(3 * ((W + 1023) / 1024 + 1) * u);
+    L.off_bsums = take(6 * 1024 * u);                  // per-CTA partials of the cooperative branching-plan kernel (<= 1024 CTAs)
     L.off_mult = take(W * sizeof(int32_t));
     L.off_donor = take(W * sizeof(int64_t));
     L.off_reclist = take(W * sizeof(int64_t));
     L.off_scalars = take(8 * u);
+    L.off_ctl = take(32 * d);
+    L.off_blockout = take(3 * kSelfcoolBlocks * d);
     L.total = off;
     return L;
 }
@@ -139,6 +142,44 @@ static bool tilt_spectrum(const sail_handle *h, const std::vector<double> &omega
     return true;
 }
 
+int check_anneal_params(sail_handle *h, const sail_anneal_params *p)
+{
+    if (!(p->eta > 0.0 && p->eta < 1.0)) return set_err(h, SAIL_ERR_ARG, "eta must be in (0, 1)");
+    if (p->amp_mode != 0 && p->amp_mode != 1) return set_err(h, SAIL_ERR_ARG, "amp_mode must be 0 or 1");
+    if (p->amp_mode == 1 && !(p->amp_p > 0.0 && p->amp_p <= 1.0 && p->amp_m > 0.0 && p->y_min > 0.0 && p->y_min <= 1.0))
+        return set_err(h, SAIL_ERR_ARG, "Eq. 30 parameters out of range");
+    if (p->trace && !(p->trace_lo >= 0 && p->trace_lo <= p->trace_hi && p->trace_hi <= h->W))
+        return set_err(h, SAIL_ERR_ARG, "trace range outside [0, W]");
+    if (p->resync_every < 0) return set_err(h, SAIL_ERR_ARG, "resync_every < 0");
+    if (p->reserved0 != 0 || p->reserved != 0) return set_err(h, SAIL_ERR_ARG, "reserved fields of sail_anneal_params must be 0");
+    return SAIL_OK;
+}
+
+// n sweeps with the temperatures d_T[0..n) already on the device: one persistent sweep-kernel launch per piece between
+// full-residual resyncs (every resync_every-th absolute sweep)
+int anneal_device_schedule(sail_handle *h, const double *d_T, int64_t n, const sail_anneal_params *p, int64_t sweeps_in_call,
+                           int64_t call_offset)
+{
+    int64_t done = 0;
+    while (done < n) {
+        int64_t chunk = n - done;
+        if (p->resync_every > 0) {
+            const int64_t to_boundary = p->resync_every - (h->sweep % p->resync_every);
+            if (to_boundary < chunk) chunk = to_boundary;
+        }
+        if (chunk > (1 << 30)) chunk = 1 << 30;
+        int rc = launch_sweeps(h, d_T + done, chunk, p, sweeps_in_call, call_offset + done);
+        if (rc) return rc;
+        h->sweep += chunk;
+        done += chunk;
+        if (p->resync_every > 0 && (h->sweep % p->resync_every) == 0) {
+            rc = launch_forward(h, 0, h->W);
+            if (rc) return rc;
+        }
+    }
+    return SAIL_OK;
+}
+
 } // namespace sail
 
 using namespace sail;
@@ -207,6 +248,7 @@ int sail_create(sail_t **out, const double *omega, int32_t n_omega, const double
     h->br.block_sums = U(L.off_bsums); h->br.mult = (int32_t *)(base + L.off_mult);
     h->br.donor_of = (int64_t *)(base + L.off_donor); h->br.rec_list = (int64_t *)(base + L.off_reclist);
     h->br.scalars = U(L.off_scalars);
+    h->ctl = D(L.off_ctl); h->block_out = D(L.off_blockout);
 
     int rc;
     if ((rc = stage_upload(h, D(L.off_omega), omega, n_omega * sizeof(double)))) return fail(rc);
@@ -265,42 +307,20 @@ int sail_anneal(sail_t *h, const double *T_schedule, int64_t n_sweeps, const sai
     if (!h) return SAIL_ERR_ARG;
     if (!h->initialised) return set_err(h, SAIL_ERR_STATE, "sail_anneal before sail_init_walkers");
     if (!T_schedule || !p || n_sweeps < 0) return set_err(h, SAIL_ERR_ARG, "NULL schedule/params or negative n_sweeps");
-    if (!(p->eta > 0.0 && p->eta < 1.0)) return set_err(h, SAIL_ERR_ARG, "eta must be in (0, 1)");
-    if (p->amp_mode != 0 && p->amp_mode != 1) return set_err(h, SAIL_ERR_ARG, "amp_mode must be 0 or 1");
-    if (p->amp_mode == 1 && !(p->amp_p > 0.0 && p->amp_p <= 1.0 && p->amp_m > 0.0 && p->y_min > 0.0 && p->y_min <= 1.0))
-        return set_err(h, SAIL_ERR_ARG, "Eq. 30 parameters out of range");
-    if (p->trace && !(p->trace_lo >= 0 && p->trace_lo <= p->trace_hi && p->trace_hi <= h->W))
-        return set_err(h, SAIL_ERR_ARG, "trace range outside [0, W]");
-    if (p->resync_every < 0) return set_err(h, SAIL_ERR_ARG, "resync_every < 0");
-    if (p->reserved0 != 0 || p->reserved != 0) return set_err(h, SAIL_ERR_ARG, "reserved fields of sail_anneal_params must be 0");
+    { const int rcp = check_anneal_params(h, p); if (rcp) return rcp; }
     for (int64_t i = 0; i < n_sweeps; ++i)
         if (!(T_schedule[i] > 0.0)) return set_err(h, SAIL_ERR_ARG, "T_schedule[%lld] must be > 0", (long long)i);
     if (n_sweeps == 0) return SAIL_OK;
     SAIL_CUDA_OK(h, cudaSetDevice(h->device));
     // the schedule lives in a fixed slice of the workspace (no allocation, no cudaFree at destroy: cudaFree costs up to
     // hundreds of ms on a busy context); longer schedules go through it piece by piece, stream-ordered
-    int64_t done = 0, piece_lo = 0, piece_hi = 0;
+    int64_t done = 0;
     while (done < n_sweeps) {
-        if (done == piece_hi) {
-            piece_lo = done;
-            piece_hi = done + (int64_t)h->d_T_cap < n_sweeps ? done + (int64_t)h->d_T_cap : n_sweeps;
-            SAIL_CUDA_OK(h, cudaMemcpyAsync(h->d_T, T_schedule + piece_lo, (size_t)(piece_hi - piece_lo) * sizeof(double),
-                                            cudaMemcpyHostToDevice, h->stream));
-        }
-        int64_t chunk = piece_hi - done;
-        if (p->resync_every > 0) {
-            const int64_t to_boundary = p->resync_every - (h->sweep % p->resync_every);
-            if (to_boundary < chunk) chunk = to_boundary;
-        }
-        if (chunk > (1 << 30)) chunk = 1 << 30;
-        int rc = launch_sweeps(h, h->d_T + (done - piece_lo), chunk, p, n_sweeps, done);
+        const int64_t piece = done + (int64_t)h->d_T_cap < n_sweeps ? (int64_t)h->d_T_cap : n_sweeps - done;
+        SAIL_CUDA_OK(h, cudaMemcpyAsync(h->d_T, T_schedule + done, (size_t)piece * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+        int rc = anneal_device_schedule(h, h->d_T, piece, p, n_sweeps, done);
         if (rc) return rc;
-        h->sweep += chunk;
-        done += chunk;
-        if (p->resync_every > 0 && (h->sweep % p->resync_every) == 0) {
-            rc = launch_forward(h, 0, h->W);
-            if (rc) return rc;
-        }
+        done += piece;
     }
     return SAIL_OK;
 }
@@ -342,15 +362,13 @@ int sail_branch_fraction(sail_t *h, double fraction, double t_imprint, double *T
     if (!(fraction >= 0.0 && fraction < 1.0) || !(t_imprint >= 0.0 && t_imprint <= 1.0))
         return set_err(h, SAIL_ERR_ARG, "need 0 <= fraction < 1 and 0 <= t <= 1");
     SAIL_CUDA_OK(h, cudaSetDevice(h->device));
-    double T = 0.0;
-    int rc = launch_branch_fraction(h, fraction, t_imprint, &T);
+    int rc = launch_branch_fraction(h, fraction, t_imprint);
     if (rc) return rc;
-    if (T_found) *T_found = T;
-    if (T == 0.0) {                                     // no event: degenerate population or nothing asked for
-        if (info) { info->n_recipients = 0; info->max_multiplier = 1; info->reserved = 0; info->chi2_min = 0.0; }
-        if (mult_out) for (int64_t i = 0; i < h->W; ++i) mult_out[i] = 1;
-        if (donor_out) for (int64_t i = 0; i < h->W; ++i) donor_out[i] = -1;
-        return SAIL_OK;
+    if (T_found) {
+        unsigned long long bits = 0;
+        SAIL_CUDA_OK(h, cudaMemcpyAsync(&bits, h->br.scalars + 5, 8, cudaMemcpyDeviceToHost, h->stream));
+        SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
+        memcpy(T_found, &bits, 8);                  // 0 = no event (degenerate population, or fraction W rounds to 0)
     }
     return branch_outputs(h, info, mult_out, donor_out);
 }

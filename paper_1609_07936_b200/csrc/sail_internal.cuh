@@ -12,6 +12,7 @@
 
 namespace sail {
 
+constexpr int kSelfcoolBlocksMax = 4096;   // blocks of the self-cooling protocol whose (T, chi2_ave, chi2_min) are kept on the device per pass
 constexpr int kMaxTau = 512;        // 32 lanes x 16 tau-points per lane (register-resident residual)
 constexpr int kMaxOmega = 8192;     // sweep-kernel tables (ratio, 1/(k domega), start values) + proposal records fit 227 KB of shared memory
 
@@ -48,7 +49,7 @@ struct BranchScratch {
     int32_t *mult;               // [W]
     int64_t *donor_of;           // [W]
     int64_t *rec_list;           // [W] recipient indices in ascending order
-    unsigned long long *scalars; // [8]: 0 chi2_min bits, 1 S, 2 n_rec, 3 max_mult
+    unsigned long long *scalars; // [8]: 0 chi2_min (ordered key), 1 S, 2 n_rec, 3 max_mult, 4 (chi2 statistics), 5 T used (double bits), 6-7 scratch
 };
 
 } // namespace sail
@@ -75,6 +76,7 @@ struct sail_handle {
     sail::BranchScratch br{};
     // sweep-kernel tables (built by the first sail_anneal)
     bool tables_ready = false;
+    int plan_ctas = 0;           // grid of the cooperative branching-plan kernel (all CTAs co-resident)
     bool tables_fact = false;
     int fact_shift = 0;
     double *sw_ratio = nullptr;  // [n_omega] exp(-omega_k G dtau)
@@ -82,6 +84,8 @@ struct sail_handle {
     double *sw_E0 = nullptr;     // direct: [n_omega][G]; factored: H[n_hi][G] then L[n_lo][G]
     double *d_T = nullptr;       // device copy of the schedule piece in flight (a fixed slice of the workspace)
     size_t d_T_cap = 0;
+    double *ctl = nullptr;             // [32] device control block: 0 T, 1 branching fraction, 2 imprint strength (branch.cu), 8.. self-cooling state (selfcool.cu)
+    double *block_out = nullptr;       // [3][kSelfcoolBlocksMax] T, chi2_ave, chi2_min per block of the self-cooling protocol
     double *model_scratch = nullptr;   // [max_walkers][n_tau]: sail_get_model's scaled copy M = c mt for the host
 
     int64_t launches = 0;
@@ -143,8 +147,12 @@ int launch_problem_tables(sail_handle *h, const double *d_F, const double *d_sig
 int launch_forward(sail_handle *h, int64_t w0, int64_t n);            // mt, chi2 of walkers [w0, w0+n)
 int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sail_anneal_params *p,
                   int64_t sweeps_in_call, int64_t call_offset);
+int check_anneal_params(sail_handle *h, const sail_anneal_params *p);
+int anneal_device_schedule(sail_handle *h, const double *d_T, int64_t n, const sail_anneal_params *p, int64_t sweeps_in_call,
+                           int64_t call_offset);
 int launch_branch(sail_handle *h, double T, double t_imprint);
-int launch_branch_fraction(sail_handle *h, double fraction, double t_imprint, double *T_found);   // row f2
+int launch_branch_fraction(sail_handle *h, double fraction, double t_imprint);                     // row f2; T found -> scalars[5]
+int launch_branch_ctl(sail_handle *h, bool by_fraction, const double *ctl);                         // (T, fraction, t) on the device
 int launch_smooth(sail_handle *h, double s);                          // Eq. 27-29 + renormalisation + forward
 int launch_scale_model(sail_handle *h, double *dst);                  // dst[w][j] = c_j mt[w][j]
 int ensure_sweep_tables(sail_handle *h);

@@ -3,14 +3,18 @@
 // reached: T = 10 starting residues for block 0 (:216), T = chi2_ave while "boiling", a linear ramp to chi2_min,
 // then a freeze-out below chi2_min that falls like 1 / steps (:162).  A block is sweeps_per_block sweeps at that T,
 // the smoothing step (if asked for) and one imprinted-branching event (:218-220).
-// The statistics are two kernels with a fixed summation order (bit-reproducible run to run); the rule itself is
-// scalar host arithmetic on their two results, as in the paper's own driver.
+// The whole feedback loop stays on the device: the statistics (two kernels with a fixed summation order, bit-reproducible
+// run to run), the rule (one thread), the block's schedule slice, the acceptance-driven strength (reading B7) and the
+// parameters of the branching event live in the handle's control block; the host only enqueues.  T / chi2_ave /
+// chi2_min per block come back once at the end of the call.
 #include "sail_internal.cuh"
-#include <vector>
 
 namespace sail {
 
 constexpr int kStatBlocks = 256, kStatThreads = 256;
+// control block (h->ctl): 0 T of the block, 1 branching fraction, 2 imprint strength (read by branch.cu);
+// 8 chi2_min, 9 chi2_ave (statistics); 10 chi2_0; 11 largest block acceptance rate so far; 12 error flag
+constexpr int kCtlT = 0, kCtlFrac = 1, kCtlImp = 2, kCtlMin = 8, kCtlAve = 9, kCtlChi0 = 10, kCtlAccMax = 11, kCtlErr = 12;
 
 // partial[b] = sum of chi2[i] over i = b * 256 + t + k * (blocks * 256), added per thread in increasing i, then over
 // the threads of the block in a fixed tree; pmin[b] likewise
@@ -44,7 +48,8 @@ __global__ void chi2_stats_final_kernel(int blocks, long long W, const double *p
     out[1] = s / (double)W;
 }
 
-int launch_chi2_stats(sail_handle *h, double *host_min, double *host_mean)
+// (chi2_min, chi2_ave) of the population -> ctl[8], ctl[9]; stream-ordered, no host access
+static int enqueue_chi2_stats(sail_handle *h)
 {
     const long long W = h->W;
     int blocks = (int)((W + kStatThreads - 1) / kStatThreads);
@@ -52,13 +57,19 @@ int launch_chi2_stats(sail_handle *h, double *host_min, double *host_mean)
     if (blocks > W / 2) blocks = (int)(W / 2 > 0 ? W / 2 : 1);          // partial sums and minima share scanA [W]
     double *partial = reinterpret_cast<double *>(h->br.scanA);
     double *pmin = W >= 2 ? partial + blocks : reinterpret_cast<double *>(h->br.scanB);
-    double *out = reinterpret_cast<double *>(h->br.scalars + 4);
     chi2_stats_partial_kernel<<<blocks, kStatThreads, 0, h->stream>>>(W, h->st.chi2, partial, pmin);
     SAIL_LAUNCH_OK(h, "chi2_stats_partial_kernel");
-    chi2_stats_final_kernel<<<1, 1, 0, h->stream>>>(blocks, W, partial, pmin, out);
+    chi2_stats_final_kernel<<<1, 1, 0, h->stream>>>(blocks, W, partial, pmin, h->ctl + kCtlMin);
     SAIL_LAUNCH_OK(h, "chi2_stats_final_kernel");
+    return SAIL_OK;
+}
+
+int launch_chi2_stats(sail_handle *h, double *host_min, double *host_mean)
+{
+    int rc = enqueue_chi2_stats(h);
+    if (rc) return rc;
     double res[2];
-    SAIL_CUDA_OK(h, cudaMemcpyAsync(res, out, sizeof res, cudaMemcpyDeviceToHost, h->stream));
+    SAIL_CUDA_OK(h, cudaMemcpyAsync(res, h->ctl + kCtlMin, sizeof res, cudaMemcpyDeviceToHost, h->stream));
     SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
     if (host_min) *host_min = res[0];
     if (host_mean) *host_mean = res[1];
@@ -75,26 +86,53 @@ __global__ void sum_u64_kernel(long long W, const unsigned long long *__restrict
     if ((threadIdx.x & 31) == 0) atomicAdd(dst, s);
 }
 
-static int accepted_total(sail_handle *h, unsigned long long *total)
+// scalars[6] <- sum of the accepted-move counters (scalars[7] keeps the previous total)
+static int enqueue_accepted_total(sail_handle *h)
 {
-    unsigned long long *dst = h->br.scalars + 7;
+    unsigned long long *dst = h->br.scalars + 6;
     SAIL_CUDA_OK(h, cudaMemsetAsync(dst, 0, 8, h->stream));
     const int blocks = (int)((h->W + 255) / 256 < 256 ? (h->W + 255) / 256 : 256);
     sum_u64_kernel<<<blocks, 256, 0, h->stream>>>(h->W, h->st.n_acc, dst);
     SAIL_LAUNCH_OK(h, "sum_u64_kernel");
-    SAIL_CUDA_OK(h, cudaMemcpyAsync(total, dst, 8, cudaMemcpyDeviceToHost, h->stream));
-    SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
     return SAIL_OK;
 }
 
-// readings C1-C3: the temperature of block b from the residues measured before it
-static double selfcool_T(int64_t b, double chi2_0, double ave, double mn, const sail_selfcool_params *p)
+struct CoolRule { int n_boil, n_ramp; double T_start, freeze_rate, t_imprint, fraction; };
+
+// readings C1-C3: the temperature of block b from the residues measured before it (ctl[8], ctl[9]); fills the block's
+// schedule slice, the branching parameters and the per-block outputs.  One thread.
+__global__ void selfcool_rule_kernel(long long b, int out_slot, CoolRule r, int has_override, double T_override, int k,
+                                     double *ctl, double *d_T, double *block_out, int out_stride)
 {
-    if (b == 0) return p->T_start * chi2_0;
-    if (b <= p->n_boil) return ave;
-    if (b <= (int64_t)p->n_boil + p->n_ramp) return ave + (mn - ave) * ((double)(b - p->n_boil) / (double)p->n_ramp);
-    return mn / (1.0 + p->freeze_rate * (double)(b - p->n_boil - p->n_ramp));
+    const double mn = ctl[kCtlMin], ave = ctl[kCtlAve];
+    if (b == 0) { ctl[kCtlChi0] = ave; ctl[kCtlAccMax] = 0.0; }   // the unit of T and of the residue (:216)
+    double T;
+    if (has_override) T = T_override;
+    else if (b == 0) T = r.T_start * ctl[kCtlChi0];
+    else if (b <= r.n_boil) T = ave;
+    else if (b <= (long long)r.n_boil + r.n_ramp) T = ave + (mn - ave) * ((double)(b - r.n_boil) / (double)r.n_ramp);
+    else T = mn / (1.0 + r.freeze_rate * (double)(b - r.n_boil - r.n_ramp));
+    if (!(T > 0.0)) { ctl[kCtlErr] = 1.0 + (double)b; T = 1.0; }   // reported by the host at the end of the call
+    for (int i = 0; i < k; ++i) d_T[i] = T;
+    ctl[kCtlT] = T; ctl[kCtlFrac] = r.fraction; ctl[kCtlImp] = r.t_imprint;
+    block_out[out_slot] = T; block_out[out_stride + out_slot] = ave; block_out[2 * out_stride + out_slot] = mn;
 }
+
+// :184 (reading B7): less imprinting and a smaller branching fraction as the acceptance rate falls — both are
+// multiplied by (acceptance rate of the block's sweeps) / (largest block acceptance rate so far); the rate is an exact
+// integer count over W k N_omega
+__global__ void selfcool_strength_kernel(double moves_per_block, CoolRule r, unsigned long long *scalars, double *ctl)
+{
+    const unsigned long long now = scalars[6], prev = scalars[7];
+    scalars[7] = now;
+    const double rate = (double)(now - prev) / moves_per_block;
+    if (rate > ctl[kCtlAccMax]) ctl[kCtlAccMax] = rate;
+    const double scale = ctl[kCtlAccMax] > 0.0 ? rate / ctl[kCtlAccMax] : 0.0;
+    ctl[kCtlFrac] = r.fraction * scale;
+    ctl[kCtlImp] = r.t_imprint * scale;
+}
+
+__global__ void copy_u64_kernel(const unsigned long long *src, unsigned long long *dst) { *dst = *src; }
 
 } // namespace sail
 
@@ -117,39 +155,48 @@ int sail_anneal_selfcool(sail_t *h, const sail_selfcool_params *p, int64_t n_blo
     if (n_blocks < 0 || p->sweeps_per_block < 1 || p->n_boil < 0 || p->n_ramp < 1 || !(p->T_start > 0.0) || !(p->freeze_rate > 0.0) ||
         !(p->t_imprint >= 0.0 && p->t_imprint <= 1.0) || !(p->smooth_s >= 0.0 && p->smooth_s <= 0.5) || !(p->branch_fraction >= 0.0 && p->branch_fraction < 1.0))
         return set_err(h, SAIL_ERR_ARG, "bad self-cooling parameters");
+    if ((size_t)p->sweeps_per_block > h->d_T_cap) return set_err(h, SAIL_ERR_ARG, "sweeps_per_block > %zu", h->d_T_cap);
+    if (p->anneal.trace || p->anneal.flags)
+        return set_err(h, SAIL_ERR_ARG, "sail_anneal_selfcool does not trace (trace and flags of the anneal parameters must be NULL)");
+    { const int rcp = check_anneal_params(h, &p->anneal); if (rcp) return rcp; }
+    if (p->T_override)
+        for (int64_t b = 0; b < n_blocks; ++b)
+            if (!(p->T_override[b] > 0.0)) return set_err(h, SAIL_ERR_ARG, "T_override[%lld] must be > 0", (long long)b);
     SAIL_CUDA_OK(h, cudaSetDevice(h->device));
-    double chi2_0 = 0.0, acc_max = 0.0;
-    unsigned long long acc_prev = 0ull;
-    if (p->adapt) { int rc0 = accepted_total(h, &acc_prev); if (rc0) return rc0; }
-    std::vector<double> T((size_t)p->sweeps_per_block);
-    for (int64_t b = 0; b < n_blocks; ++b) {
-        double mn = 0.0, ave = 0.0;
-        int rc = launch_chi2_stats(h, &mn, &ave);
-        if (rc) return rc;
-        if (b == 0) chi2_0 = ave;                        // the unit of T and of the residue (:216)
-        const double Tb = p->T_override ? p->T_override[b] : selfcool_T(b, chi2_0, ave, mn, p);
-        if (!(Tb > 0.0)) return set_err(h, SAIL_ERR_ARG, "self-cooling reached T = %g at block %lld", Tb, (long long)b);
-        if (T_out) T_out[b] = Tb;
-        if (chi2_ave_out) chi2_ave_out[b] = ave;
-        if (chi2_min_out) chi2_min_out[b] = mn;
-        for (auto &x : T) x = Tb;
-        if ((rc = sail_anneal(h, T.data(), p->sweeps_per_block, &p->anneal))) return rc;
-        if (p->smooth_s > 0.0 && (rc = sail_smooth(h, p->smooth_s))) return rc;
-        // :184 (reading B7): less imprinting and a smaller branching fraction as the acceptance rate falls
-        double scale = 1.0;
-        if (p->adapt) {
-            unsigned long long acc_now = 0ull;
-            if ((rc = accepted_total(h, &acc_now))) return rc;
-            const double rate = (double)(acc_now - acc_prev) / ((double)h->W * (double)p->sweeps_per_block * (double)h->n_omega);
-            acc_prev = acc_now;
-            if (rate > acc_max) acc_max = rate;
-            scale = acc_max > 0.0 ? rate / acc_max : 0.0;
+    const CoolRule rule{p->n_boil, p->n_ramp, p->T_start, p->freeze_rate, p->t_imprint, p->branch_fraction};
+    const double moves_per_block = (double)h->W * (double)p->sweeps_per_block * (double)h->n_omega;
+    const int k = p->sweeps_per_block;
+    SAIL_CUDA_OK(h, cudaMemsetAsync(h->ctl + kCtlErr, 0, sizeof(double), h->stream));
+    int rc;
+    if (p->adapt) {                                      // scalars[7] = accepted moves so far
+        if ((rc = enqueue_accepted_total(h))) return rc;
+        copy_u64_kernel<<<1, 1, 0, h->stream>>>(h->br.scalars + 6, h->br.scalars + 7);
+        SAIL_LAUNCH_OK(h, "copy_u64_kernel");
+    }
+    for (int64_t b0 = 0; b0 < n_blocks; b0 += kSelfcoolBlocksMax) {
+        const int64_t nb = n_blocks - b0 < kSelfcoolBlocksMax ? n_blocks - b0 : kSelfcoolBlocksMax;
+        for (int64_t b = b0; b < b0 + nb; ++b) {
+            if ((rc = enqueue_chi2_stats(h))) return rc;
+            selfcool_rule_kernel<<<1, 1, 0, h->stream>>>(b, (int)(b - b0), rule, p->T_override ? 1 : 0, p->T_override ? p->T_override[b] : 0.0, k,
+                                                         h->ctl, h->d_T, h->block_out, kSelfcoolBlocksMax);
+            SAIL_LAUNCH_OK(h, "selfcool_rule_kernel");
+            if ((rc = anneal_device_schedule(h, h->d_T, k, &p->anneal, k, 0))) return rc;
+            if (p->smooth_s > 0.0 && (rc = launch_smooth(h, p->smooth_s))) return rc;
+            if (p->adapt) {
+                if ((rc = enqueue_accepted_total(h))) return rc;
+                selfcool_strength_kernel<<<1, 1, 0, h->stream>>>(moves_per_block, rule, h->br.scalars, h->ctl);
+                SAIL_LAUNCH_OK(h, "selfcool_strength_kernel");
+            }
+            if (p->branch && (rc = launch_branch_ctl(h, p->branch_fraction > 0.0, h->ctl))) return rc;
         }
-        if (p->branch) {
-            if (p->branch_fraction > 0.0) rc = sail_branch_fraction(h, p->branch_fraction * scale, p->t_imprint * scale, nullptr, nullptr, nullptr, nullptr);
-            else rc = sail_branch(h, Tb, p->t_imprint * scale, nullptr, nullptr, nullptr);
-            if (rc) return rc;
-        }
+        // one read-back per pass of up to 4096 blocks: the trajectory and the error flag
+        double err = 0.0;
+        if (T_out) SAIL_CUDA_OK(h, cudaMemcpyAsync(T_out + b0, h->block_out, (size_t)nb * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        if (chi2_ave_out) SAIL_CUDA_OK(h, cudaMemcpyAsync(chi2_ave_out + b0, h->block_out + kSelfcoolBlocksMax, (size_t)nb * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        if (chi2_min_out) SAIL_CUDA_OK(h, cudaMemcpyAsync(chi2_min_out + b0, h->block_out + 2 * kSelfcoolBlocksMax, (size_t)nb * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+        SAIL_CUDA_OK(h, cudaMemcpyAsync(&err, h->ctl + kCtlErr, sizeof err, cudaMemcpyDeviceToHost, h->stream));
+        SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
+        if (err != 0.0) return set_err(h, SAIL_ERR_ARG, "self-cooling reached T <= 0 at block %lld", (long long)(err - 1.0));
     }
     return SAIL_OK;
 }
