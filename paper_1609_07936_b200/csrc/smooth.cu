@@ -4,63 +4,61 @@
 // tilt a_k (1 + kappa (w^m_k - wbar)) about the new mean frequency, kappa = (B - B') / sum a_k (w^m_k - wbar)^2,
 // clamped so that no coefficient turns negative.
 // One WARP per walker row, no block barrier on the path: lane 0 streams whole rows global -> shared with the bulk-copy
-// engine (cp.async.bulk + one mbarrier per warp and stage; the next row is in flight while this one is reduced), the
-// lanes read the three taps from shared memory (bin k = lane + 32 i: conflict free), keep the smoothed row in registers,
-// reduce A', B' and then the variance by shuffles, and store the tilted row coalesced.  16 N_omega bytes of HBM traffic
+// engine (cp.async.bulk + one mbarrier per warp), the lanes read the three taps from shared memory (bin k = lane +
+// 32 i: conflict free) and keep the smoothed row in registers, so the stage is refilled with the warp's next row while
+// A', B' and the second moment are reduced by shuffles (one round) and the tilted row is stored coalesced.  16 N_omega bytes of HBM traffic
 // per walker.  The model and the residue are then refreshed by the dense forward kernel (row A7).
 #include "sail_internal.cuh"
 
 namespace sail {
 
-constexpr int kSmoothWarps = 6;
+constexpr int kSmoothWarps = 12;
 
-__device__ __forceinline__ double warp_sum_shfl(double x)
+// three sums over the warp at once (the butterflies interleave: one latency instead of three)
+__device__ __forceinline__ void warp_sum3(double &x, double &y, double &z)
 {
 #pragma unroll
-    for (int off = 16; off > 0; off >>= 1) x += __shfl_xor_sync(0xffffffffu, x, off);
-    return x;
+    for (int off = 16; off > 0; off >>= 1) {
+        x += __shfl_xor_sync(0xffffffffu, x, off);
+        y += __shfl_xor_sync(0xffffffffu, y, off);
+        z += __shfl_xor_sync(0xffffffffu, z, off);
+    }
 }
 
 template <int PER>   // bins per lane: n_omega <= 32 PER
 __global__ void __launch_bounds__(kSmoothWarps * 32) smooth_kernel(int n_omega, long long W, double s, double B, double domega,
                                                                    const double *__restrict__ omega, double *__restrict__ a)
 {
-    extern __shared__ __align__(128) unsigned char smem[];     // wm[n_pad] | per warp: 2 stages of n_pad doubles
-    __shared__ __align__(8) unsigned long long bars[kSmoothWarps][2];
+    extern __shared__ __align__(128) unsigned char smem[];     // wm[n_pad] | per warp: one stage of n_pad doubles
+    __shared__ __align__(8) unsigned long long bars[kSmoothWarps];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int n_pad = (n_omega + 1) & ~1;
     double *s_wm = reinterpret_cast<double *>(smem);
-    double *stage = s_wm + n_pad + (size_t)warp * 2 * n_pad;
+    double *row = s_wm + n_pad + (size_t)warp * n_pad;
     const double c = 1.0 - 2.0 * s, e = 1.0 - s, half = 0.5 * domega;
     const bool bulk = (n_omega & 1) == 0;                      // rows are multiples of 16 bytes: bulk copies
     for (int k = threadIdx.x; k < n_omega; k += blockDim.x) s_wm[k] = omega[k] + half;
+    const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&bars[warp]);
     if (lane == 0) {
-        for (int st = 0; st < 2; ++st)
-            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"((uint32_t)__cvta_generic_to_shared(&bars[warp][st])) : "memory");
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(bar) : "memory");
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
     __syncthreads();
     const long long stride = (long long)gridDim.x * kSmoothWarps;
-    auto fetch = [&](long long w, int st) {                    // lane 0: row w -> stage st
-        const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&bars[warp][st]);
-        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(stage + st * n_pad);
+    auto fetch = [&](long long w) {                            // lane 0: row w -> this warp's stage
+        const uint32_t dst = (uint32_t)__cvta_generic_to_shared(row);
         const uint32_t bytes = (uint32_t)n_omega * 8u;
         asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" :: "r"(bar), "r"(bytes) : "memory");
         asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
                      :: "r"(dst), "l"(a + (size_t)w * n_omega), "r"(bytes), "r"(bar) : "memory");
     };
     long long w = (long long)blockIdx.x * kSmoothWarps + warp;
-    if (bulk && lane == 0 && w < W) fetch(w, 0);
+    if (bulk && lane == 0 && w < W) fetch(w);
     int it = 0;
     for (; w < W; w += stride, ++it) {
-        const int st = it & 1;
         double *aw = a + (size_t)w * n_omega;
-        double *row = stage + st * n_pad;
         if (bulk) {
-            // the other stage was last read before the __syncwarp that ended the previous row
-            if (lane == 0 && w + stride < W) fetch(w + stride, st ^ 1);
-            const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&bars[warp][st]);
-            const uint32_t parity = (uint32_t)((it >> 1) & 1);
+            const uint32_t parity = (uint32_t)(it & 1);
             asm volatile("{\n\t.reg .pred p;\n\tWAIT_%=:\n\tmbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
                          "@p bra DONE_%=;\n\tbra WAIT_%=;\n\tDONE_%=:\n\t}" :: "r"(bar), "r"(parity) : "memory");
         } else {
@@ -68,7 +66,7 @@ __global__ void __launch_bounds__(kSmoothWarps * 32) smooth_kernel(int n_omega, 
             __syncwarp();
         }
         double nv[PER];
-        double sA = 0.0, sB = 0.0;
+        double sA = 0.0, sB = 0.0, sC = 0.0;
 #pragma unroll
         for (int i = 0; i < PER; ++i) {
             const int k = lane + 32 * i;
@@ -79,19 +77,20 @@ __global__ void __launch_bounds__(kSmoothWarps * 32) smooth_kernel(int n_omega, 
                 else if (k == 0) nv[i] = __dadd_rn(__dmul_rn(e, row[0]), __dmul_rn(s, row[1]));
                 else if (k == n_omega - 1) nv[i] = __dadd_rn(__dmul_rn(e, row[k]), __dmul_rn(s, row[k - 1]));
                 else nv[i] = __dadd_rn(__dadd_rn(__dmul_rn(s, row[k - 1]), __dmul_rn(c, row[k])), __dmul_rn(s, row[k + 1]));
+                const double wk = s_wm[k];
                 sA += nv[i];
-                sB = fma(nv[i], s_wm[k], sB);
+                sB = fma(nv[i], wk, sB);
+                sC = fma(nv[i] * wk, wk, sC);
             }
         }
-        const double A1 = warp_sum_shfl(sA), B1 = warp_sum_shfl(sB);
+        __syncwarp();
+        // the whole row now lives in registers: the stage is free, the next row streams in behind the reductions
+        if (bulk && lane == 0 && w + stride < W) fetch(w + stride);
+        warp_sum3(sA, sB, sC);
+        const double A1 = sA, B1 = sB;
         const double wbar = B1 / A1;
-        double sV = 0.0;
-#pragma unroll
-        for (int i = 0; i < PER; ++i) {
-            const int k = lane + 32 * i;
-            if (k < n_omega) { const double dw = s_wm[k] - wbar; sV = fma(nv[i] * dw, dw, sV); }
-        }
-        const double V = warp_sum_shfl(sV);
+        // sum a_k (w_k - wbar)^2 = sum a_k w_k^2 - wbar sum a_k w_k  (one reduction round instead of two)
+        const double V = fma(-wbar, B1, sC);
         double kappa = (V > 0.0) ? (B - B1) / V : 0.0;
         // positivity (reading S2): the tilt factor is linear in k, smallest at an end bin
         const double d_lo = s_wm[0] - wbar, d_hi = s_wm[n_omega - 1] - wbar;
@@ -102,7 +101,6 @@ __global__ void __launch_bounds__(kSmoothWarps * 32) smooth_kernel(int n_omega, 
             const int k = lane + 32 * i;
             if (k < n_omega) aw[k] = nv[i] * (1.0 + kappa * (s_wm[k] - wbar));
         }
-        __syncwarp();
     }
 }
 
@@ -111,7 +109,7 @@ int launch_smooth(sail_handle *h, double s)
     if (h->n_omega > 2048) return set_err(h, SAIL_ERR_ARG, "sail_smooth supports n_omega <= 2048");
     const long long W = h->W;
     const int n_pad = (h->n_omega + 1) & ~1;
-    const size_t smem = (size_t)(1 + 2 * kSmoothWarps) * n_pad * sizeof(double);
+    const size_t smem = (size_t)(1 + kSmoothWarps) * n_pad * sizeof(double);
     void (*kern)(int, long long, double, double, double, const double *, double *);
     const int per = (h->n_omega + 31) / 32;
     if (per <= 8) kern = smooth_kernel<8>;
