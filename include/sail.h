@@ -255,15 +255,20 @@ SAIL_API int sail_measure_fp64_peak(int32_t device, void *stream, double *dfma_p
 
 /*
  * sail_microbench — issue rates and latencies of the units the sweep kernel (rows A2-A6) leans on, measured on
- * `device` with one CTA per SM (DESIGN.md 6.1 cites them).  `out` is a HOST array of n_out >= SAIL_MICROBENCH_N
- * doubles, filled as (clk = the device's maximum SM clock):
- *   [0] DFMA warp-instructions / clk / SM at 8 warps per sub-partition   [1] DMMA m8n8k4 / clk / SM
- *   [2] clk per SM for (2 DMMA + 8 DFMA) issued together: 2/[1] + 8/[0] means DMMA has no pipe of its own
- *   [3] SHFL / clk / SM   [4] LDS.128, one address per warp, / clk / SM   [5] LDS.64, lane-contiguous, / clk / SM
- *   [6] [7] [8] dependent-issue latency of DFMA, SHFL, DMMA in clk       [9] as [0] at ONE warp per sub-partition
+ * `device` with one CTA per SM; every kernel times itself in SM cycles (clock64), so the figures are per SM clock
+ * (DESIGN.md 6.1 cites them).  `out` is a HOST array of n_out >= SAIL_MICROBENCH_N doubles:
+ *   warp-instructions / clk / SM at 4 warps per sub-partition (2.0 = one per 2 clk per sub-partition = 64 lanes):
+ *   [0] DMUL, two vector-register operands              [1] DFMA with one constant-bank operand
+ *   [2] DFMA, three vector operands, two of them shared with the neighbouring instructions (operand reuse)
+ *   [3] DFMA, three distinct vector operands            [4] DMMA m8n8k4
+ *   [5] clk per SM for (2 DMMA + 8 DFMA) issued together: 2/[4] + 8/[2] means DMMA has no pipe of its own
+ *   [6] SHFL   [7] LDS.128, one address per warp   [8] LDS.64, lane-contiguous
+ *   [9] [10] [11] dependent-issue latency of DFMA, SHFL, DMMA in clk   [12] as [2] at ONE warp per sub-partition
+ *   [13] the sweep kernel's tau loop alone (C = 16, 12 warps per SM): CREDITED (5 per tau-point) warp-instr / clk / SM
+ *   [14] [15] latency in clk of the warp sum by 2 DMMA + DADD / by the 5-stage fp64 shuffle butterfly
  * Returns SAIL_ERR_ARG for a NULL / short array, SAIL_ERR_CUDA without a device.
  */
-#define SAIL_MICROBENCH_N 10
+#define SAIL_MICROBENCH_N 16
 SAIL_API int sail_microbench(int32_t device, void *stream, double *out, int32_t n_out);
 
 #ifdef __cplusplus

@@ -115,9 +115,11 @@ def measure_fp64_peak(device=0):
     return out.value
 
 
-MICROBENCH_KEYS = ("dfma_per_clk_sm", "dmma_m8n8k4_per_clk_sm", "clk_per_sm_2dmma_8dfma", "shfl_per_clk_sm",
+MICROBENCH_KEYS = ("dmul_2op_per_clk_sm", "dfma_const_operand_per_clk_sm", "dfma_3op_reuse_per_clk_sm", "dfma_3op_distinct_per_clk_sm",
+                   "dmma_m8n8k4_per_clk_sm", "clk_per_sm_2dmma_8dfma", "shfl_per_clk_sm",
                    "lds128_uniform_per_clk_sm", "lds64_lane_per_clk_sm", "dfma_latency_clk", "shfl_latency_clk",
-                   "dmma_latency_clk", "dfma_per_clk_sm_1warp_per_subpartition")
+                   "dmma_latency_clk", "dfma_3op_reuse_per_clk_sm_1warp_per_subpartition", "tau_loop_credited_per_clk_sm",
+                   "warp_sum_dmma_latency_clk", "warp_sum_shfl_latency_clk")
 
 
 def microbench(device=0):

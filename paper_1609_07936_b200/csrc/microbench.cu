@@ -1,94 +1,164 @@
 // microbench.cu — sail_microbench: the per-SM issue rates and latencies the sweep-kernel design rests on
 // (DESIGN.md §6.1), measured on the device the library runs on.  Diagnostics only; not part of the method.
-//   FP64 FMA rate, DMMA m8n8k4 rate alone and mixed with DFMA (do they share a pipe?), warp-shuffle rate,
-//   broadcast and per-lane shared-memory load rates, and the dependent-issue latencies of DFMA / SHFL / DMMA.
+// Every kernel times itself with clock64() (SM cycles between its first and last instruction, averaged over the CTAs,
+// one CTA per SM), so the figures are per SM clock whatever the clock is and carry no launch overhead.
+// The central finding (profiles/r02_fp64_pipe.md): an FP64 instruction occupies the FP64 pipe of a sub-partition for
+// max(2, number of 64-bit VECTOR-register operands it must read) cycles — DADD / DMUL / DFMA with a constant-bank or
+// uniform operand issue at 0.5 per clock per sub-partition, a DFMA with three distinct vector operands at 0.333, a DFMA
+// whose consecutive neighbours share two of its operands (reuse cache) at 0.444.
 #include "sail_internal.cuh"
 
 namespace sail {
 
-constexpr int kUbIter = 4096;
+constexpr int kUbIter = 2048;
 
 #define SAIL_DMMA(c0, c1, a, b)                                                                              \
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"         \
                  : "+d"(c0), "+d"(c1) : "d"(a), "d"(b))
 
-// MODE 0: 8 independent DFMA chains   1: 4 independent DMMA chains   2: 2 DMMA + 8 DFMA interleaved
-//      3: 8 independent SHFL          4: LDS.128, one address for the whole warp
-//      5: LDS.64, lane-contiguous     6: dependent DFMA   7: dependent SHFL   8: dependent DMMA
+struct UbParams { double a, b; };
+
+// MODE 0: x = y_u * x_u (DMUL, two vector operands)       1: x = fma(x, P.a, y_u) (one constant-bank operand)
+//      2: x = fma(x, a, b) (a, b reused by the neighbours)  3: x_u = fma(y_u, z_u, x_u) (three distinct vector operands)
+//      4: 4 independent DMMA chains   5: 2 DMMA + 8 DFMA (mode 2 form) interleaved   6: 8 independent SHFL
+//      7: LDS.128, one address for the whole warp   8: LDS.64, lane-contiguous
+//      9: dependent DFMA   10: dependent SHFL   11: dependent DMMA
+//     12: DMMA warp sum (2 DMMA + DADD), dependent   13: 5-stage fp64 shuffle butterfly, dependent
 template <int MODE>
-__global__ void ub_kernel(double a, double b, double *sink)
+__global__ void __launch_bounds__(512) ub_kernel(const UbParams P, const double *init, double *sink, long long *clk_out)
 {
     __shared__ __align__(16) double sm[512];
     for (int i = threadIdx.x; i < 512; i += blockDim.x) sm[i] = (double)i;
     __syncthreads();
-    double x0 = threadIdx.x, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    double x[8], y[8], z[8];
+#pragma unroll
+    for (int u = 0; u < 8; ++u) { x[u] = init[threadIdx.x + 32 * u]; y[u] = init[300 + threadIdx.x + 32 * u]; z[u] = init[600 + threadIdx.x + 32 * u]; }
+    const double a = init[1000], b = init[1001];
     int s0 = threadIdx.x, s1 = s0 * 3, s2 = s0 * 5, s3 = s0 * 7, s4 = s0 + 11, s5 = s0 + 13, s6 = s0 + 17, s7 = s0 + 19;
-    const uint32_t base = (uint32_t)__cvta_generic_to_shared(sm) + ((MODE == 5) ? (threadIdx.x & 31) * 8 : 0);
+    const uint32_t base = (uint32_t)__cvta_generic_to_shared(sm) + ((MODE == 8) ? (threadIdx.x & 31) * 8 : 0);
+    const double one = 1.0, zero = 0.0;
+    const long long t0 = clock64();
 #pragma unroll 1
     for (int i = 0; i < kUbIter; ++i) {
-        if (MODE == 0) {
-            x0 = fma(x0, a, b); x1 = fma(x1, a, b); x2 = fma(x2, a, b); x3 = fma(x3, a, b);
-            x4 = fma(x4, a, b); x5 = fma(x5, a, b); x6 = fma(x6, a, b); x7 = fma(x7, a, b);
-        } else if (MODE == 1) {
-            SAIL_DMMA(x0, x1, a, b); SAIL_DMMA(x2, x3, a, b); SAIL_DMMA(x4, x5, a, b); SAIL_DMMA(x6, x7, a, b);
-        } else if (MODE == 2) {
-            double y0 = x0, y1 = x1;
-            SAIL_DMMA(y0, y1, a, b); x0 = y0; x1 = y1;
-            x2 = fma(x2, a, b); x3 = fma(x3, a, b); x4 = fma(x4, a, b); x5 = fma(x5, a, b);
-            double z0 = x6, z1 = x7;
-            SAIL_DMMA(z0, z1, a, b); x6 = z0; x7 = z1;
-            x2 = fma(x2, a, b); x3 = fma(x3, a, b); x4 = fma(x4, a, b); x5 = fma(x5, a, b);
-        } else if (MODE == 3) {
+        if (MODE <= 3) {
+#pragma unroll
+            for (int r = 0; r < 2; ++r)
+#pragma unroll
+                for (int u = 0; u < 8; ++u) {
+                    if (MODE == 0) x[u] = y[u] * x[u];
+                    else if (MODE == 1) x[u] = fma(x[u], P.a, y[u]);
+                    else if (MODE == 2) x[u] = fma(x[u], a, b);
+                    else x[u] = fma(y[u], z[u], x[u]);
+                }
+        } else if (MODE == 4) {
+            SAIL_DMMA(x[0], x[1], a, b); SAIL_DMMA(x[2], x[3], a, b); SAIL_DMMA(x[4], x[5], a, b); SAIL_DMMA(x[6], x[7], a, b);
+        } else if (MODE == 5) {
+            SAIL_DMMA(x[0], x[1], a, b);
+            x[2] = fma(x[2], a, b); x[3] = fma(x[3], a, b); x[4] = fma(x[4], a, b); x[5] = fma(x[5], a, b);
+            SAIL_DMMA(x[6], x[7], a, b);
+            x[2] = fma(x[2], a, b); x[3] = fma(x[3], a, b); x[4] = fma(x[4], a, b); x[5] = fma(x[5], a, b);
+        } else if (MODE == 6) {
             s0 = __shfl_xor_sync(0xffffffffu, s0, 1); s1 = __shfl_xor_sync(0xffffffffu, s1, 2);
             s2 = __shfl_xor_sync(0xffffffffu, s2, 4); s3 = __shfl_xor_sync(0xffffffffu, s3, 8);
             s4 = __shfl_xor_sync(0xffffffffu, s4, 16); s5 = __shfl_xor_sync(0xffffffffu, s5, 1);
             s6 = __shfl_xor_sync(0xffffffffu, s6, 2); s7 = __shfl_xor_sync(0xffffffffu, s7, 4);
-        } else if (MODE == 4 || MODE == 5) {
+        } else if (MODE == 7 || MODE == 8) {
 #pragma unroll
             for (int u = 0; u < 8; ++u) {           // the address depends on i; results are folded with integer ops
-                const uint32_t ad = base + (uint32_t)(((i + u) & 7) * ((MODE == 4) ? 16 : 256));
+                const uint32_t ad = base + (uint32_t)(((i + u) & 7) * ((MODE == 7) ? 16 : 256));
                 unsigned long long p, q = 0ull;
-                if (MODE == 4) asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(p), "=l"(q) : "r"(ad));
+                if (MODE == 7) asm volatile("ld.shared.v2.b64 {%0,%1}, [%2];" : "=l"(p), "=l"(q) : "r"(ad));
                 else           asm volatile("ld.shared.b64 %0, [%1];" : "=l"(p) : "r"(ad));
                 s0 ^= (int)(p ^ q); s1 ^= (int)((p ^ q) >> 32);
             }
-        } else if (MODE == 6) {
+        } else if (MODE == 9) {
 #pragma unroll
-            for (int u = 0; u < 8; ++u) x0 = fma(x0, a, b);
-        } else if (MODE == 7) {
+            for (int u = 0; u < 8; ++u) x[0] = fma(x[0], a, b);
+        } else if (MODE == 10) {
 #pragma unroll
             for (int u = 0; u < 8; ++u) s0 = __shfl_xor_sync(0xffffffffu, s0, 1 << (u & 3));
+        } else if (MODE == 11) {
+#pragma unroll
+            for (int u = 0; u < 4; ++u) SAIL_DMMA(x[0], x[1], a, b);
+        } else if (MODE == 12) {
+            double c0, c1, t0d, t1d;
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%4,%4};" : "=d"(c0), "=d"(c1) : "d"(one), "d"(x[0]), "d"(zero));
+            const double h = c0 + c1;
+            asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%4,%4};" : "=d"(t0d), "=d"(t1d) : "d"(one), "d"(h), "d"(zero));
+            x[0] = t0d;
         } else {
 #pragma unroll
-            for (int u = 0; u < 4; ++u) SAIL_DMMA(x0, x1, a, b);
+            for (int off = 16; off > 0; off >>= 1) x[0] += __shfl_xor_sync(0xffffffffu, x[0], off);
         }
     }
-    const double r = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7 + (double)(s0 + s1 + s2 + s3 + s4 + s5 + s6 + s7);
+    const long long t1 = clock64();
+    if (threadIdx.x == 0) clk_out[blockIdx.x] = t1 - t0;
+    double r = 0.0;
+#pragma unroll
+    for (int u = 0; u < 8; ++u) r += x[u] + y[u] + z[u];
+    r += (double)(s0 + s1 + s2 + s3 + s4 + s5 + s6 + s7);
     if (r == 123.456) *sink = r;
 }
 
-template <int MODE>
-static double ub_cycles_per_instr(cudaStream_t st, int blocks, int threads, double instr_per_iter, double clock_hz, double *sink,
-                                  bool per_sm)
+// the tau loop of the sweep kernel on its own (C = 16 tau-points per lane, the order ptxas picks for the kernel: the
+// recurrence, then d, then t and the accumulation; d kept for the accepted update), one "move" after the other from
+// the same registers: what the FP64 pipe delivers on the credited 5 instructions per tau-point when nothing else runs
+__global__ void __launch_bounds__(384) ub_tau_kernel(const double *init, double *sink, long long *clk_out)
 {
-    cudaEvent_t e0, e1;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    ub_kernel<MODE><<<blocks, threads, 0, st>>>(1.0000001, 1e-9, sink);
-    float best = 1e30f;
-    for (int rep = 0; rep < 3; ++rep) {
-        cudaEventRecord(e0, st);
-        ub_kernel<MODE><<<blocks, threads, 0, st>>>(1.0000001, 1e-9, sink);
-        cudaEventRecord(e1, st);
-        cudaEventSynchronize(e1);
-        float ms = 0.f;
-        cudaEventElapsedTime(&ms, e0, e1);
-        if (ms < best) best = ms;
+    constexpr int C = 16;
+    double mt[C], G2[C], Wt[C], d[C];
+#pragma unroll
+    for (int i = 0; i < C; ++i) { mt[i] = init[threadIdx.x % 256 + 32 * i]; G2[i] = init[1024 + threadIdx.x % 256 + 32 * i]; Wt[i] = init[2048 + threadIdx.x % 256 + 32 * i]; d[i] = 0.0; }
+    double alpha = init[3000], sx = init[3001], sy = init[3002], v0 = init[3003 + (threadIdx.x & 31)], v1 = init[3040 + (threadIdx.x & 31)];
+    double total = 0.0;
+    const long long t0 = clock64();
+#pragma unroll 1
+    for (int m = 0; m < kUbIter; ++m) {
+        double vm = v0, vc = v1, acc_a = 0.0, acc_b = 0.0;
+#pragma unroll
+        for (int i = 0; i < C; ++i) {
+            double vi;
+            if (i == 0) vi = vm;
+            else if (i == 1) vi = vc;
+            else { vi = fma(sx, vc, sy * vm); vm = vc; vc = vi; }
+            d[i] = fma(alpha, mt[i], vi);
+            const double t = fma(Wt[i], d[i], G2[i]);
+            if (i & 1) acc_b = fma(d[i], t, acc_b);
+            else       acc_a = fma(d[i], t, acc_a);
+        }
+        const double s = acc_a + acc_b;
+        total += s;
+        alpha = fma(s, 1e-300, alpha);
+        v0 = fma(s, 1e-300, v0);
+        if (s == 1.2345) {                          // never: keeps d[] alive like the accepted branch of the kernel
+#pragma unroll
+            for (int i = 0; i < C; ++i) { mt[i] += d[i]; G2[i] = fma(Wt[i], d[i] + d[i], G2[i]); }
+        }
     }
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    const double cycles = best * 1e-3 * clock_hz;
-    const double warps_per_sm = threads / 32.0;        // one CTA per SM
-    const double instr = kUbIter * instr_per_iter * (per_sm ? warps_per_sm : 1.0);
-    return cycles / instr;                              // cycles per warp-instruction (per SM, or per warp)
+    const long long t1 = clock64();
+    if (threadIdx.x == 0) clk_out[blockIdx.x] = t1 - t0;
+    if (total == 1.2345) sink[0] = total + mt[0] + G2[C - 1];
+}
+
+struct UbCtx { cudaStream_t st; int sms; UbParams P; double *init, *sink; long long *clk; };
+
+// average SM cycles of one launch (second of two: the first warms the instruction cache)
+template <typename Launch>
+static double ub_cycles(const UbCtx &c, Launch launch)
+{
+    long long h[1024];
+    for (int rep = 0; rep < 2; ++rep) launch();
+    cudaMemcpyAsync(h, c.clk, (size_t)c.sms * sizeof(long long), cudaMemcpyDeviceToHost, c.st);
+    cudaStreamSynchronize(c.st);
+    double avg = 0.0;
+    for (int i = 0; i < c.sms; ++i) avg += (double)h[i];
+    return avg / c.sms;
+}
+
+template <int MODE>
+static double ub_run(const UbCtx &c, int threads)
+{
+    return ub_cycles(c, [&] { ub_kernel<MODE><<<c.sms, threads, 0, c.st>>>(c.P, c.init, c.sink, c.clk); });
 }
 
 } // namespace sail
@@ -102,25 +172,42 @@ int sail_microbench(int32_t device, void *stream, double *out, int32_t n_out)
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || device < 0 || device >= ndev) { cudaGetLastError(); return set_err(nullptr, SAIL_ERR_CUDA, "no usable CUDA device"); }
     if (cudaSetDevice(device) != cudaSuccess) return set_err(nullptr, SAIL_ERR_CUDA, "cudaSetDevice failed");
-    int sms = 0, khz = 0;
-    cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, device);
-    cudaDeviceGetAttribute(&khz, cudaDevAttrClockRate, device);
-    const double hz = khz * 1e3;
-    cudaStream_t st = (cudaStream_t)stream;
-    double *sink = nullptr;
-    if (cudaMalloc(&sink, 8) != cudaSuccess) return set_err(nullptr, SAIL_ERR_ALLOC, "cudaMalloc failed");
-    const int T = 32 * 32;                              // 8 warps per sub-partition
-    out[0] = 1.0 / ub_cycles_per_instr<0>(st, sms, T, 8, hz, sink, true);     // DFMA warp-instr / clk / SM
-    out[1] = 1.0 / ub_cycles_per_instr<1>(st, sms, T, 4, hz, sink, true);     // DMMA m8n8k4 / clk / SM
-    out[2] = ub_cycles_per_instr<2>(st, sms, T, 1, hz, sink, true);           // cycles per SM for 2 DMMA + 8 DFMA
-    out[3] = 1.0 / ub_cycles_per_instr<3>(st, sms, T, 8, hz, sink, true);     // SHFL / clk / SM
-    out[4] = 1.0 / ub_cycles_per_instr<4>(st, sms, T, 8, hz, sink, true);     // LDS.128 (uniform address) / clk / SM
-    out[5] = 1.0 / ub_cycles_per_instr<5>(st, sms, T, 8, hz, sink, true);     // LDS.64 (lane-contiguous) / clk / SM
-    out[6] = ub_cycles_per_instr<6>(st, sms, 32, 8, hz, sink, false);         // dependent DFMA latency, cycles
-    out[7] = ub_cycles_per_instr<7>(st, sms, 32, 8, hz, sink, false);         // dependent SHFL latency, cycles
-    out[8] = ub_cycles_per_instr<8>(st, sms, 32, 4, hz, sink, false);         // dependent DMMA latency, cycles
-    out[9] = 1.0 / ub_cycles_per_instr<0>(st, sms, 4 * 32, 8, hz, sink, true); // DFMA / clk / SM at ONE warp per sub-partition
-    cudaFree(sink);
+    UbCtx c{};
+    cudaDeviceGetAttribute(&c.sms, cudaDevAttrMultiProcessorCount, device);
+    if (c.sms > 1024) c.sms = 1024;
+    c.st = (cudaStream_t)stream;
+    c.P = UbParams{1.0000001, 1e-9};
+    char *buf = nullptr;
+    const size_t n_init = 4096;
+    if (cudaMalloc(&buf, n_init * 8 + 64 + 1024 * 8) != cudaSuccess) { cudaGetLastError(); return set_err(nullptr, SAIL_ERR_ALLOC, "cudaMalloc failed"); }
+    c.init = (double *)buf; c.sink = (double *)(buf + n_init * 8); c.clk = (long long *)(buf + n_init * 8 + 64);
+    {
+        double h[n_init];
+        for (size_t i = 0; i < n_init; ++i) h[i] = 1.0 + 1e-9 * (double)(i % 97);
+        h[1000] = 1.0000001; h[1001] = 1e-9;
+        h[3000] = -1e-3; h[3001] = 1.9; h[3002] = -0.9;
+        cudaMemcpyAsync(c.init, h, sizeof h, cudaMemcpyHostToDevice, c.st);
+        cudaStreamSynchronize(c.st);
+    }
+    const int T8 = 16 * 32;                                  // 4 warps per sub-partition (the rates saturate from 2)
+    const double w8 = T8 / 32.0, it = (double)kUbIter;
+    out[0] = it * 16 * w8 / ub_run<0>(c, T8);                // DMUL (2 vector operands), warp-instr / clk / SM
+    out[1] = it * 16 * w8 / ub_run<1>(c, T8);                // DFMA, one constant-bank operand
+    out[2] = it * 16 * w8 / ub_run<2>(c, T8);                // DFMA, 3 vector operands, 2 reused by the neighbours
+    out[3] = it * 16 * w8 / ub_run<3>(c, T8);                // DFMA, 3 distinct vector operands
+    out[4] = it * 4 * w8 / ub_run<4>(c, T8);                 // DMMA m8n8k4 / clk / SM
+    out[5] = ub_run<5>(c, T8) / (it * w8);                   // clk per SM for (2 DMMA + 8 DFMA)
+    out[6] = it * 8 * w8 / ub_run<6>(c, T8);                 // SHFL / clk / SM
+    out[7] = it * 8 * w8 / ub_run<7>(c, T8);                 // LDS.128 (uniform address) / clk / SM
+    out[8] = it * 8 * w8 / ub_run<8>(c, T8);                 // LDS.64 (lane-contiguous) / clk / SM
+    out[9] = ub_run<9>(c, 32) / (it * 8);                    // dependent DFMA latency, clk
+    out[10] = ub_run<10>(c, 32) / (it * 8);                  // dependent SHFL latency, clk
+    out[11] = ub_run<11>(c, 32) / (it * 4);                  // dependent DMMA latency, clk
+    out[12] = it * 16 * 4 / ub_run<2>(c, 4 * 32);            // mode 2 at ONE warp per sub-partition, warp-instr / clk / SM
+    out[13] = it * 80 * 12 / ub_cycles(c, [&] { ub_tau_kernel<<<c.sms, 384, 0, c.st>>>(c.init, c.sink, c.clk); });   // credited warp-instr / clk / SM
+    out[14] = ub_run<12>(c, 32) / it;                        // DMMA warp sum latency, clk
+    out[15] = ub_run<13>(c, 32) / it;                        // shuffle-butterfly warp sum latency, clk
+    cudaFree(buf);
     cudaError_t e = cudaGetLastError();
     if (e != cudaSuccess) return set_err(nullptr, SAIL_ERR_CUDA, "microbenchmark failed: %s", cudaGetErrorString(e));
     return SAIL_OK;

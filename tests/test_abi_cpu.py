@@ -83,11 +83,11 @@ def test_no_cpu_fallback_without_a_device(lib):
         binding.Sail(omega, tau, F, max_walkers=4)
     out = C.c_double()
     assert lib.sail_measure_fp64_peak(0, None, C.byref(out)) == binding.SAIL_ERR_CUDA
-    buf = (C.c_double * 10)()
+    buf = (C.c_double * 16)()
     lib.sail_microbench.argtypes = [C.c_int32, C.c_void_p, C.POINTER(C.c_double), C.c_int32]
-    assert lib.sail_microbench(0, None, buf, 10) == binding.SAIL_ERR_CUDA
+    assert lib.sail_microbench(0, None, buf, 16) == binding.SAIL_ERR_CUDA
     assert lib.sail_microbench(0, None, buf, 3) == binding.SAIL_ERR_ARG          # array too short
-    assert lib.sail_microbench(0, None, None, 10) == binding.SAIL_ERR_ARG
+    assert lib.sail_microbench(0, None, None, 16) == binding.SAIL_ERR_ARG
     lib.sail_smooth.argtypes = [C.c_void_p, C.c_double]
     assert lib.sail_smooth(None, 0.02) == binding.SAIL_ERR_ARG
     assert lib.sail_destroy(None) == 0
