@@ -237,6 +237,21 @@ SAIL_API int sail_stats(sail_t *h, int64_t *accepted, int64_t *evaluated, double
 SAIL_API int sail_set_walkers(sail_t *h, int64_t w0, int64_t n, const double *spectra, const double *y);
 SAIL_API int sail_set_sweep(sail_t *h, int64_t sweep);
 
+/*
+ * sail_set_chi2 — overwrite the RUNNING residues chi2_0 + sum dchi2 of walkers [w0, w0+n) with HOST values (resuming
+ * from a checkpoint restores the running sums bit for bit, sail_set_walkers recomputes them from the spectra; the
+ * parity tests use it to give both sides identical weights input).  The model is not touched.  Synchronises.
+ */
+SAIL_API int sail_set_chi2(sail_t *h, int64_t w0, int64_t n, const double *chi2);
+
+/*
+ * sail_set_walker_offset — global index of this handle's walker 0 (default 0).  The Philox counter of a move is
+ * (global walker index, sweep, move, stream), so a population split over several handles (one per GPU: contiguous walker
+ * ranges, paper_1609_07936_b200/distributed.py) draws exactly the random numbers of the single-handle run.  Branching
+ * stays per handle.  offset + max_walkers must be < 2^32.
+ */
+SAIL_API int sail_set_walker_offset(sail_t *h, int64_t first_walker);
+
 /* sail_destroy — free library-owned memory (never the caller's workspace).  NULL is OK. */
 SAIL_API int sail_destroy(sail_t *h);
 

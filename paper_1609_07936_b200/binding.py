@@ -18,7 +18,7 @@ SAIL_OK, SAIL_ERR_ARG, SAIL_ERR_GRID, SAIL_ERR_ALLOC, SAIL_ERR_CUDA, SAIL_ERR_ST
 
 EXPORTS = ["sail_workspace_bytes", "sail_create", "sail_init_walkers", "sail_anneal", "sail_branch",
            "sail_resync", "sail_get", "sail_get_model", "sail_stats", "sail_set_walkers", "sail_set_sweep",
-           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak", "sail_microbench", "sail_smooth", "sail_chi2_stats", "sail_anneal_selfcool", "sail_branch_fraction"]
+           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak", "sail_microbench", "sail_smooth", "sail_chi2_stats", "sail_anneal_selfcool", "sail_branch_fraction", "sail_set_walker_offset", "sail_set_chi2"]
 
 
 class SailError(RuntimeError):
@@ -86,6 +86,8 @@ def lib():
         L.sail_stats.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_void_p]
         L.sail_set_walkers.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p, C.c_void_p]
         L.sail_set_sweep.argtypes = [C.c_void_p, C.c_int64]
+        L.sail_set_walker_offset.argtypes = [C.c_void_p, C.c_int64]
+        L.sail_set_chi2.argtypes = [C.c_void_p, C.c_int64, C.c_int64, C.c_void_p]
         L.sail_destroy.argtypes = [C.c_void_p]
         L.sail_last_error.restype = C.c_char_p
         L.sail_last_error.argtypes = [C.c_void_p]
@@ -285,6 +287,15 @@ class Sail:
         sp = _f64(spectra).reshape(-1, self.n_omega)
         yy = _f64(y) if y is not None else None
         self._check(self._L.sail_set_walkers(self._h, w0, sp.shape[0], _ptr(sp), _ptr(yy)))
+
+    def set_chi2(self, chi2, w0=0):
+        """Overwrite the running residues of walkers [w0, w0 + len(chi2))."""
+        c2 = _f64(chi2)
+        self._check(self._L.sail_set_chi2(self._h, w0, c2.size, _ptr(c2)))
+
+    def set_walker_offset(self, first_walker):
+        """Global index of walker 0: sharded populations draw the single-handle random streams."""
+        self._check(self._L.sail_set_walker_offset(self._h, first_walker))
 
     def set_sweep(self, sweep):
         self._check(self._L.sail_set_sweep(self._h, sweep))

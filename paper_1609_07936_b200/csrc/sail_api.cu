@@ -446,6 +446,25 @@ int sail_set_walkers(sail_t *h, int64_t w0, int64_t n, const double *spectra, co
     return SAIL_OK;
 }
 
+int sail_set_chi2(sail_t *h, int64_t w0, int64_t n, const double *chi2)
+{
+    if (!h) return SAIL_ERR_ARG;
+    if (!h->initialised) return set_err(h, SAIL_ERR_STATE, "sail_set_chi2 before sail_init_walkers");
+    if (!chi2 || w0 < 0 || n < 0 || w0 + n > h->W) return set_err(h, SAIL_ERR_ARG, "bad walker range or NULL chi2");
+    SAIL_CUDA_OK(h, cudaSetDevice(h->device));
+    SAIL_CUDA_OK(h, cudaMemcpyAsync(h->st.chi2 + w0, chi2, (size_t)n * sizeof(double), cudaMemcpyHostToDevice, h->stream));
+    SAIL_CUDA_OK(h, cudaStreamSynchronize(h->stream));
+    return SAIL_OK;
+}
+
+int sail_set_walker_offset(sail_t *h, int64_t first_walker)
+{
+    if (!h || first_walker < 0 || first_walker + h->max_walkers > (int64_t)0xFFFFFFFFll)
+        return h ? set_err(h, SAIL_ERR_ARG, "walker offset must satisfy 0 <= offset and offset + max_walkers < 2^32") : SAIL_ERR_ARG;
+    h->walker0 = first_walker;
+    return SAIL_OK;
+}
+
 int sail_set_sweep(sail_t *h, int64_t sweep)
 {
     if (!h || sweep < 0) return h ? set_err(h, SAIL_ERR_ARG, "sweep < 0") : SAIL_ERR_ARG;

@@ -65,6 +65,7 @@ struct sail_handle {
     std::vector<double> omega_host;   // the caller's omega grid (sail_create copies it)
     uint64_t seed = 0;
     int64_t sweep = 0;          // absolute sweep counter
+    int64_t walker0 = 0;        // global index of walker 0 (sail_set_walker_offset)
     bool initialised = false;
 
     void *workspace = nullptr;  // base of everything below

@@ -144,6 +144,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
             walk_src = s_spec;
             __syncwarp();
         }
+        const uint32_t wid = (uint32_t)(w + P.walker0);      // Philox counter word 0: the GLOBAL walker index
         double chi2 = P.chi2[w];
         double g = 1.0, ginv = 1.0;
         bool tracing = false;
@@ -166,22 +167,22 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                 Draw dr{0, 0, 0.0};
                 int wl = 0;                                        // WALK: steps this lane's move walks
                 if (lane < nb) {
-                    dr = draw_move(P, (uint32_t)w, sweep_abs, (uint32_t)(m0 + lane), y_sweep, T_sweep, my_rec_w);
+                    dr = draw_move(P, wid, sweep_abs, (uint32_t)(m0 + lane), y_sweep, T_sweep, my_rec_w);
                     int p = dr.p, s = dr.s_raw + (dr.s_raw >= dr.p ? 1 : 0);
                     if (WALK) {
                         wl = P.walk_len;
                         if (P.walk_uniform > 0.0) {                // :158 uniform admixture: this move keeps its uniform indices
                             uint32_t xm[4];
-                            philox4x32_10((uint32_t)w, sweep_abs, (uint32_t)(m0 + lane), (uint32_t)(2 + P.walk_len), P.seed_lo, P.seed_hi, xm);
+                            philox4x32_10(wid, sweep_abs, (uint32_t)(m0 + lane), (uint32_t)(2 + P.walk_len), P.seed_lo, P.seed_hi, xm);
                             if (u01(xm[0]) < P.walk_uniform) wl = 0;
                         }
 #pragma unroll
                         for (int l = 0; l < 2; ++l) {
                             uint32_t xw[4] = {0u, 0u, 0u, 0u};
-                            if (l < wl) philox4x32_10((uint32_t)w, sweep_abs, (uint32_t)(m0 + lane), (uint32_t)(2 + l), P.seed_lo, P.seed_hi, xw);
+                            if (l < wl) philox4x32_10(wid, sweep_abs, (uint32_t)(m0 + lane), (uint32_t)(2 + l), P.seed_lo, P.seed_hi, xw);
                             *reinterpret_cast<uint4 *>(my_rec_w + 80 + 16 * l) = make_uint4(xw[0], xw[1], xw[2], xw[3]);
                         }
-                        index_walk(P, (uint32_t)w, sweep_abs, (uint32_t)(m0 + lane), wl, my_rec_w, walk_src, p, dr.s_raw, s);
+                        index_walk(P, wid, sweep_abs, (uint32_t)(m0 + lane), wl, my_rec_w, walk_src, p, dr.s_raw, s);
                     }
                     write_indexed(P, p, s, dr.alpha, s_ratio, s_invd, wm(s), wm(p), my_rec_w);
                 }
@@ -283,7 +284,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                             if (((behind >> lane) & 1u) && wl > 0) {
                                 const int2 q = *reinterpret_cast<const int2 *>(my_rec_w);
                                 int p = dr.p, s = q.y;
-                                index_walk(P, (uint32_t)w, sweep_abs, (uint32_t)(m0 + lane), wl, my_rec_w, walk_src, p, dr.s_raw, s);
+                                index_walk(P, wid, sweep_abs, (uint32_t)(m0 + lane), wl, my_rec_w, walk_src, p, dr.s_raw, s);
                                 if (p != q.x || s != q.y) write_indexed(P, p, s, dr.alpha, s_ratio, s_invd, wm(s), wm(p), my_rec_w);
                             }
                             __syncwarp();
@@ -470,7 +471,7 @@ int launch_sweeps(sail_handle *h, const double *d_T, int64_t n_sweeps, const sai
         return set_err(h, SAIL_ERR_ARG, "W * n_omega must be < 2^32 spectral coefficients");
 
     SweepArgs a{};
-    a.n_omega = h->n_omega; a.n_tau = h->n_tau; a.W = h->W;
+    a.n_omega = h->n_omega; a.n_tau = h->n_tau; a.W = h->W; a.walker0 = h->walker0;
     a.A = h->A; a.B = h->B; a.domega = h->domega; a.eta = p->eta;
     a.amp_p = p->amp_p; a.amp_m = p->amp_m; a.y_min = p->y_min; a.amp_mode = p->amp_mode;
     a.seed_lo = (uint32_t)(h->seed & 0xFFFFFFFFu); a.seed_hi = (uint32_t)(h->seed >> 32);

@@ -8,6 +8,7 @@ namespace sail {
 struct SweepArgs {
     int n_omega, n_tau;
     long long W;
+    long long walker0;                 // global index of this handle's walker 0 (Philox counter word 0)
     double A, B, domega, eta, amp_p, amp_m, y_min;
     int amp_mode;
     uint32_t seed_lo, seed_hi;
