@@ -347,6 +347,18 @@ def main_ours(args):
     sdist.barrier(dev)
     clocks = sampler.stop()
     chi2_final = chi2_t.cpu().numpy()
+    if args.profile_sweeps:
+        # the target of the ncu captures under profiles/: walkers re-initialised, sweeps [0, S) of the schedule in one
+        # launch (no branching), then ONE short launch of N sweeps at sweep S = --profile-at (default: mid-anneal).
+        # ncu: `-k regex:sweep_kernel -s <launches before> -c 1`; a whole block is seconds long and far too slow to replay
+        at = args.profile_at if args.profile_at >= 0 else w.n_sweeps // 2
+        at = max(0, min(at, w.n_sweeps - args.profile_sweeps))
+        s.init_walkers(w.W, w.A, w.B, seed)
+        if at:
+            s.anneal(w.schedule[:at], **dict(anneal_params(w), resync_every=0))
+        torch.cuda.synchronize()
+        s.anneal(w.schedule[at:at + args.profile_sweeps], **dict(anneal_params(w), resync_every=0))
+        torch.cuda.synchronize()
     step_moves = w.W * bs * w.n_omega
     total_s, total_moves = sdist.reduce_timing(float(np.sum(step_s)), float(step_moves * args.steps), dev)
     value = total_moves / total_s
@@ -583,6 +595,8 @@ if __name__ == "__main__":
     ap.add_argument("--e2e", type=int, default=-1, help="steps of the end-to-end (host buffers) run; -1 = as many as --steps, 0 = skip")
     ap.add_argument("--configs", type=int, default=1, help="also run one whole anneal of each BASELINE.json configuration (N=1 only)")
     ap.add_argument("--extra", type=int, default=1, help="also time resync / smoothing / branching / walk rows and the microbenchmarks (N=1 only)")
+    ap.add_argument("--profile-sweeps", type=int, default=0, help="after the timed steps: re-init, anneal to --profile-at, then one launch of N sweeps (ncu target)")
+    ap.add_argument("--profile-at", type=int, default=-1, help="sweep index of the --profile-sweeps launch (-1 = mid-anneal)")
     ap.add_argument("--selfcool", type=int, default=0, help="run N blocks of the paper's self-cooling protocol instead of the bench (supplementary)")
     ap.add_argument("--noise-sweep", action="store_true", help="run BASELINE.json configs[3] as configured (4 eps x --noise-reps anneals)")
     ap.add_argument("--noise-reps", type=int, default=8)

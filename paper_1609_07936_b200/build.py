@@ -1,6 +1,9 @@
 """Build libsail_b200.so (the C-ABI product library) in-tree with nvcc for sm_100a.
 
-    python -m paper_1609_07936_b200.build [--force] [--verbose]
+    python -m paper_1609_07936_b200.build [--force] [--verbose] [--define NAME=VALUE ...]
+
+`--define` passes -DNAME=VALUE to nvcc for every source (diagnostic builds, e.g. SAIL_DIAG_EXTRA_DFMA in csrc/sweep.cu);
+it always recompiles, and a later plain build restores the product library (the defines are recorded in build/defines.txt).
 
 Cross-compiles without a GPU.  The .so is git-ignored but travels to the GPU box with the snapshot.
 """
@@ -35,8 +38,20 @@ def _stale(target, deps):
     return any(os.path.getmtime(d) > t for d in deps)
 
 
-def build(force: bool = False, verbose: bool = False) -> str:
+def build(force: bool = False, verbose: bool = False, defines=None) -> str:
+    """defines = None: keep the -D flags of the library that is there (bench.py on a diagnostic build);
+    defines = () : the product library; defines = ["NAME=VALUE", ...]: a diagnostic build."""
     os.makedirs(OBJ, exist_ok=True)
+    # a library built with other -D flags than the ones asked for now is stale, whatever the time stamps say
+    stamp = os.path.join(OBJ, "defines.txt")
+    have = open(stamp).read() if os.path.exists(stamp) else ""
+    if defines is None:
+        defines = have.split()
+    want = " ".join(sorted(defines))
+    if want != have:
+        force = True
+    with open(stamp, "w") as f:
+        f.write(want)
     headers = [os.path.join(CSRC, f) for f in os.listdir(CSRC) if f.endswith((".cuh", ".h"))]
     headers.append(os.path.join(INCLUDE, "sail.h"))
     nvcc = _nvcc()
@@ -47,7 +62,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
         o = os.path.join(OBJ, src.replace(".cu", ".o"))
         objs.append(o)
         if force or _stale(o, [s] + headers):
-            cmd = [nvcc] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-c", s, "-o", o]
+            cmd = [nvcc] + NVCC_FLAGS + ["-D" + d for d in defines] + (["-Xptxas", "-v"] if verbose else []) + ["-I", INCLUDE, "-c", s, "-o", o]
             jobs.append(cmd)
 
     def run(cmd):
@@ -65,4 +80,5 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv))
+    defs = [sys.argv[i + 1] for i, a in enumerate(sys.argv[:-1]) if a == "--define"]
+    print(build(force="--force" in sys.argv, verbose="--verbose" in sys.argv, defines=defs))

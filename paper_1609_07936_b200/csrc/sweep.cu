@@ -31,6 +31,14 @@
 //           against the two changed bins); the Philox words of the first two steps are staged behind the record.
 #include "sweep_common.cuh"
 
+// Diagnostic, off by default (no code): SAIL_DIAG_EXTRA_DFMA = N adds N FP64 instructions per evaluated move on two
+// chains that nothing in the move depends on.  If the kernel had latency slack they would be free; measured, each costs
+// 0.6-0.9 clk per SM per move, i.e. at least its own FP64-pipe time (profiles/r02_sweep_pipe_bound.md).
+// Build with `python -m paper_1609_07936_b200.build --force --define SAIL_DIAG_EXTRA_DFMA=8`.
+#ifndef SAIL_DIAG_EXTRA_DFMA
+#define SAIL_DIAG_EXTRA_DFMA 0
+#endif
+
 namespace sail {
 
 // state-independent half of a proposal (row A2): Philox -> uniform p, s (reading G11), rho, -T ln u, 1/rho
@@ -146,6 +154,9 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
         }
         const uint32_t wid = (uint32_t)(w + P.walker0);      // Philox counter word 0: the GLOBAL walker index
         double chi2 = P.chi2[w];
+#if SAIL_DIAG_EXTRA_DFMA > 0
+        double diag_a = 0.5, diag_b = 0.25;
+#endif
         double g = 1.0, ginv = 1.0;
         bool tracing = false;
         if (TRACE) tracing = P.trace != nullptr && w >= P.trace_lo && w < P.trace_hi;
@@ -246,6 +257,13 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                         if (i & 1) acc_b = fma(d[i], t, acc_b);
                         else       acc_a = fma(d[i], t, acc_a);
                     }
+#if SAIL_DIAG_EXTRA_DFMA > 0
+#pragma unroll
+                    for (int q = 0; q < SAIL_DIAG_EXTRA_DFMA; ++q) {
+                        if (q & 1) diag_b = fma(diag_b, alpha, th.x);
+                        else       diag_a = fma(diag_a, alpha, th.x);
+                    }
+#endif
                     const double dchi2 = warp_sum_dmma((C > 1) ? acc_a + acc_b : acc_a);
                     ev_mask |= 1u << m;
                     if (TRACE) { if (lane == m) tr_dchi2 = dchi2; }
@@ -335,6 +353,9 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
             const int j = lane + G * i;
             if (j < P.n_tau) P.mt[(size_t)w * P.n_tau + j] = mt[i];
         }
+#if SAIL_DIAG_EXTRA_DFMA > 0
+        if (diag_a + diag_b == 1.2345) chi2 += 1.0;           // never: keeps the two chains alive
+#endif
         if (lane == 0) P.chi2[w] = chi2;
         __syncwarp();
     }

@@ -14,7 +14,7 @@ ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
 @pytest.fixture(scope="module")
 def lib():
     from paper_1609_07936_b200 import build, binding
-    build.build()
+    build.build(defines=())
     return binding.lib()
 
 
