@@ -43,15 +43,12 @@ FP64_LANES_PER_SM = 64          # FP64 lanes per SM per clock (4 sub-partitions 
 DFMA_PER_TAU_POINT = 5          # algorithmic FP64-pipe instructions per tau-point per evaluated move
 NAMES = ["tiny", "small", "branching", "noise", "stress"]
 
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep-kernel launch as bench.py issues it (whole anneal for tiny /
-# small, one block of branch_every sweeps otherwise), from the committed `ncu --set full` captures
-# (profiles/r02_sweep_dram_bytes.json names the capture of every entry)
-SWEEP_DRAM_BYTES_PER_LAUNCH = {"small": 15.13e6}
-try:
-    with open(os.path.join(ROOT, "profiles", "r02_sweep_dram_bytes.json")) as _f:
-        SWEEP_DRAM_BYTES_PER_LAUNCH.update({k: v for k, v in json.load(_f).items() if not k.startswith("_")})
-except Exception:
-    pass
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep-kernel launch, from the committed `ncu --set full` captures
+# profiles/r02_sweep_{stress,noise,small}_full_metrics.txt (2-sweep launches).  A warp runs ALL sweeps of a launch on a
+# walker while that walker's spectrum and model are resident on chip, so the DRAM traffic of a launch is the walker state
+# once in and once out (algorithmic: 16 W (N_omega + N_tau) bytes) whatever the number of sweeps; states that fit the
+# 126 MB L2 (small, noise) partly stay there between launches.
+SWEEP_DRAM_BYTES_PER_LAUNCH = {"stress": 11.094e9, "noise": 0.2822e9, "small": 11.9e6}
 
 
 # ------------------------------------------------------------------------------------------------
@@ -383,6 +380,17 @@ def main_ours(args):
                     "launch_ms": 1e3 * kern_total / max(args.steps, 1),
                     "evaluated_moves_per_s": evaluated / kern_total,
                     "evaluated_fraction": evaluated / attempted, "accepted_fraction": accepted / attempted}
+        try:
+            # what the FP64 pipe delivers on the credited instructions alone (the tau loop with nothing else running,
+            # `sail_microbench`): its three-operand DFMAs are operand-fetch bound (profiles/r02_sweep_pipe_bound.md)
+            from paper_1609_07936_b200.binding import microbench
+            mb = microbench(local_rank)
+            loop_peak = mb["tau_loop_credited_per_clk_sm"] * 32 * num_sms * sm_max * 1e6
+            roofline["credited_loop_alone"] = {"warp_instr_per_clk_sm": mb["tau_loop_credited_per_clk_sm"], "rate": loop_peak / 1e12,
+                                               "unit": "T FP64 lane-instr/s", "frac_of_nominal": loop_peak / peak_nominal,
+                                               "kernel_frac_of_it": achieved / loop_peak}
+        except Exception as ex:  # supplementary only
+            roofline["credited_loop_alone"] = {"error": repr(ex)}
 
         # ---- end to end through the C ABI with host buffers: the same K steps --------------------------------
         e2e = None
