@@ -186,12 +186,14 @@ __global__ void __launch_bounds__(kPlanThreads) branch_plan_kernel(const PlanArg
 
     // ---- temperature: given, or searched (reading B6) ------------------------------------------------------------
     double T = (a.mode == 2) ? a.ctl[0] : a.T;
-    bool event = true;
+    // a population whose smallest residue is not finite (all NaN, or -inf) has no weights: every E_i would be 0 and the
+    // comb would divide by S = 0.  No event then (identical on every CTA, so the grid leaves together).
+    bool event = isfinite(cmin) && (a.mode == 1 || a.mode == 3 || T > 0.0);
     if (a.mode == 1 || a.mode == 3) {
         const double fraction = (a.mode == 3) ? a.ctl[1] : a.fraction;
         const long long n0 = (long long)floor(fraction * (double)W + 0.5);
         T = 0.0;
-        event = n0 > 0 && cmax > cmin;
+        event = event && n0 > 0 && cmax > cmin;
         if (event) {
             double lo, hi = 1.0 / (cmax - cmin);
             if ((long long)pass(1.0 / hi, false) >= n0) {

@@ -629,6 +629,25 @@ def test_branch_fraction_degenerate_population_is_a_no_op():
     s.close()
 
 
+def test_branching_on_a_population_without_finite_residues_is_a_no_op():
+    """All residues NaN (or the smallest one -inf): no weight of Eq. 24 is defined, the event must not happen — no
+    recipient, spectra untouched — for sail_branch and for sail_branch_fraction."""
+    w = wl.make("tiny", simpson_intervals=20_000)
+    W = 600
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED)
+    s.anneal(np.full(2, 0.5), w.eta)
+    a0, _ = s.get()
+    for bad in (np.full(W, np.nan), np.concatenate(([-np.inf], np.full(W - 1, 3.0)))):
+        s.set_chi2(bad)
+        info, mult, donor = s.branch(1.0, 0.5, want_maps=True)
+        assert info.n_recipients == 0 and (mult == 1).all() and (donor == -1).all()
+        T, info, _, _ = s.branch_fraction(0.25, 0.5)
+        assert info.n_recipients == 0 and T == 0.0
+        assert np.array_equal(s.get()[0], a0)
+    s.close()
+
+
 def test_schedule_longer_than_the_device_slice_is_uploaded_in_pieces():
     """sail_anneal keeps 32768 temperatures on the device at a time: a 33000-sweep call must equal the same sweeps
     issued as 32768 + 232 (absolute sweep counter, stream-ordered re-upload of the slice)."""
