@@ -28,7 +28,7 @@
 //           overflow L1: Stress);
 //   WALK    index selection by a truncated Markov walk on the current spectrum (section 2.3): every lane walks its own
 //           move at batch time, and the lanes behind an accepted move walk again (their candidates may have compared
-//           against the two changed bins); the Philox words of the first two steps are staged behind the record.
+//           against the two changed bins: only those whose walk READ one of them); the Philox words of the first two steps are staged behind the record.
 #include "sweep_common.cuh"
 
 // Diagnostic, off by default (no code): SAIL_DIAG_EXTRA_DFMA = N adds N FP64 instructions per evaluated move on two
@@ -62,8 +62,26 @@ __device__ __forceinline__ Draw draw_move(const SweepArgs &P, uint32_t walker, u
 // final p and walks L steps on those.  Step l uses Philox counter (walker, sweep, move, 2 + l) = (candidate for p,
 // u for p, candidate for s, u for s); the first two steps' words are staged at rec + 80.  The walk reads a RATIO of
 // coefficients of the current spectrum, so the lazy scale cancels.
+// The bins a walk READ (its two starts and every candidate; at most 2 L + 2): its outcome can change only if one of
+// them changes.  Eight 16-bit slots in a 128-bit shift register (n_omega <= 8192 < 0xFFFF, the empty value); a longer
+// walk sets `all` and counts as touching every bin.
+struct WalkBins {
+    unsigned long long lo, hi;
+    int n;
+    __device__ __forceinline__ void clear() { lo = hi = ~0ull; n = 0; }
+    __device__ __forceinline__ void add(int bin) { hi = (hi << 16) | (lo >> 48); lo = (lo << 16) | (unsigned long long)(unsigned)bin; ++n; }
+    __device__ __forceinline__ bool has(int bin) const
+    {
+        if (n > 8) return true;
+        const unsigned long long k = (unsigned long long)(unsigned)bin * 0x0001000100010001ull, m = 0x8000800080008000ull, o = 0x0001000100010001ull;
+        const unsigned long long x = lo ^ k, y = hi ^ k;                 // a zero 16-bit slot = a match
+        return ((((x - o) & ~x) | ((y - o) & ~y)) & m) != 0ull;
+    }
+};
+
+template <bool TRACK>
 __device__ __forceinline__ void index_walk(const SweepArgs &P, uint32_t walker, uint32_t sweep, uint32_t move, int wl,
-                                           const unsigned char *rec, const double *a_row, int &p, int s_raw, int &s)
+                                           const unsigned char *rec, const double *a_row, int &p, int s_raw, int &s, WalkBins &vis)
 {
     auto words = [&](int l, uint32_t (&xw)[4]) {
         if (l < 2) {
@@ -73,18 +91,22 @@ __device__ __forceinline__ void index_walk(const SweepArgs &P, uint32_t walker, 
             philox4x32_10(walker, sweep, move, (uint32_t)(2 + l), P.seed_lo, P.seed_hi, xw);
         }
     };
+    if (TRACK) { vis.clear(); if (wl > 0) vis.add(p); }
     for (int l = 0; l < wl; ++l) {
         uint32_t xw[4];
         words(l, xw);
         const int c = (int)__umulhi(xw[0], (uint32_t)P.n_omega);
+        if (TRACK) vis.add(c);
         if (__dmul_rn(u01(xw[1]), ld_f64(a_row + p)) < ld_f64(a_row + c)) p = c;
     }
     s = s_raw + (s_raw >= p ? 1 : 0);
+    if (TRACK && wl > 0) vis.add(s);
     for (int l = 0; l < wl; ++l) {
         uint32_t xw[4];
         words(l, xw);
         int c = (int)__umulhi(xw[2], (uint32_t)(P.n_omega - 1));
         c += (c >= p) ? 1 : 0;
+        if (TRACK) vis.add(c);
         if (__dmul_rn(u01(xw[3]), ld_f64(a_row + s)) < ld_f64(a_row + c)) s = c;
     }
 }
@@ -94,6 +116,9 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
 {
     constexpr int G = 32;
     constexpr int kRec = WALK ? kRecWalkBytes : kRecBytes;
+    // WALK: track the bins a walk read (so that only affected lanes walk again) in the kernels that have the registers
+    // for it; measured at L = 2: +10 % on a 1024-bin grid, -4 % at 256 bins in the 72-register form, which keeps re-walking
+    constexpr bool TRACK = WALK && C > 4;
     extern __shared__ __align__(16) unsigned char smem[];
     double *s_ratio = reinterpret_cast<double *>(smem);
     const int n_omega = P.n_omega;
@@ -177,6 +202,8 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                 // ---- proposals of the batch (row A2), one move per lane ------------------------------------
                 Draw dr{0, 0, 0.0};
                 int wl = 0;                                        // WALK: steps this lane's move walks
+                WalkBins vis;                                      // WALK: the bins this lane's walk read
+                vis.clear();
                 if (lane < nb) {
                     dr = draw_move(P, wid, sweep_abs, (uint32_t)(m0 + lane), y_sweep, T_sweep, my_rec_w);
                     int p = dr.p, s = dr.s_raw + (dr.s_raw >= dr.p ? 1 : 0);
@@ -193,7 +220,7 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                             if (l < wl) philox4x32_10(wid, sweep_abs, (uint32_t)(m0 + lane), (uint32_t)(2 + l), P.seed_lo, P.seed_hi, xw);
                             *reinterpret_cast<uint4 *>(my_rec_w + 80 + 16 * l) = make_uint4(xw[0], xw[1], xw[2], xw[3]);
                         }
-                        index_walk(P, wid, sweep_abs, (uint32_t)(m0 + lane), wl, my_rec_w, walk_src, p, dr.s_raw, s);
+                        index_walk<TRACK>(P, wid, sweep_abs, (uint32_t)(m0 + lane), wl, my_rec_w, walk_src, p, dr.s_raw, s, vis);
                     }
                     write_indexed(P, p, s, dr.alpha, s_ratio, s_invd, wm(s), wm(p), my_rec_w);
                 }
@@ -298,14 +325,18 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
                             __syncwarp();
                         }
                         if (WALK) {
-                            // the lanes behind the accepted move walk again on the changed spectrum
-                            if (((behind >> lane) & 1u) && wl > 0) {
-                                const int2 q = *reinterpret_cast<const int2 *>(my_rec_w);
-                                int p = dr.p, s = q.y;
-                                index_walk(P, wid, sweep_abs, (uint32_t)(m0 + lane), wl, my_rec_w, walk_src, p, dr.s_raw, s);
-                                if (p != q.x || s != q.y) write_indexed(P, p, s, dr.alpha, s_ratio, s_invd, wm(s), wm(p), my_rec_w);
+                            // the accepted move changed bins p and s: a lane behind it walks again only if its walk
+                            // READ one of the two (nothing else can change its indices); no lane, no work
+                            const bool again = ((behind >> lane) & 1u) && wl > 0 && (!TRACK || vis.has(r0.x) || vis.has(r0.y));
+                            if (__ballot_sync(0xffffffffu, again)) {
+                                if (again) {
+                                    const int2 q = *reinterpret_cast<const int2 *>(my_rec_w);
+                                    int p = dr.p, s = q.y;
+                                    index_walk<TRACK>(P, wid, sweep_abs, (uint32_t)(m0 + lane), wl, my_rec_w, walk_src, p, dr.s_raw, s, vis);
+                                    if (p != q.x || s != q.y) write_indexed(P, p, s, dr.alpha, s_ratio, s_invd, wm(s), wm(p), my_rec_w);
+                                }
+                                __syncwarp();
                             }
-                            __syncwarp();
                         }
                         // the spectrum changed: screen the moves behind this one again
                         mask = screen(behind);
