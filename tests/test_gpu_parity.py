@@ -662,7 +662,10 @@ def test_schedule_longer_than_the_device_slice_is_uploaded_in_pieces():
 
 
 @pytest.mark.parametrize("name,W,L,n_sw,mix", [("tiny", 64, 1, 20, 0.0), ("tiny", 64, 3, 20, 0.25), ("small", 45, 2, 6, 0.0),
-                                               ("stress", 9, 2, 2, 0.1)])
+                                               ("stress", 9, 2, 2, 0.1),
+                                               # the kernels that track the bins a walk read (C > 4): a 1024-bin grid, L = 3
+                                               # (the eight slots exactly full) and L = 4 (overflow: every lane walks again)
+                                               ("noise", 24, 2, 3, 0.0), ("branching", 20, 3, 3, 0.2), ("branching", 12, 4, 2, 0.0)])
 def test_index_walk_parity(name, W, L, n_sw, mix):
     """f4 (section 2.3, :156-158; reading F4): with p and s chosen by an L-step Metropolis walk on the CURRENT spectrum
     the GPU still makes the oracle's moves one for one: identical indices, rho, decisions; dchi2 within 1e-12 L1."""
@@ -683,6 +686,28 @@ def test_index_walk_parity(name, W, L, n_sw, mix):
     o0 = _oracle(w, W); o0.init_walkers(W)
     t0, _ = o0.anneal(T[:1], trace_walkers=(0, W), want_flags=True)
     assert (to["p"][:, 0] != t0["p"]).mean() > 0.05
+    s.close()
+
+
+@pytest.mark.parametrize("name,W,L", [("noise", 40, 2), ("stress", 16, 1), ("small", 60, 2)])
+def test_index_walk_untraced_end_state(name, W, L):
+    """The untraced walk binaries (the ones a run without trace buffers launches; C = 8 / 16 track the read bins of every
+    pending walk, C = 4 does not): END state against the oracle — spectra, chi^2, accepted / evaluated counters, y."""
+    w = wl.make(name, simpson_intervals=20_000)
+    o = oracle.Oracle(w.omega, w.tau, w.F, w.sigma, w.A, w.B, w.eta, SEED, walk_len=L)
+    o.init_walkers(W)
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED, spectra=o.a)
+    T = wl.geometric_schedule(1.0, 0.3, 3)
+    assert s.anneal(T, w.eta, walk_length=L) == (None, None)
+    o.anneal(T)
+    a, c2 = s.get()
+    acc, ev, y = s.stats()
+    np.testing.assert_array_equal(acc, o.acc)
+    np.testing.assert_array_equal(ev, o.feas)
+    np.testing.assert_allclose(y, o.y, rtol=1e-15, atol=0)
+    np.testing.assert_allclose(a, o.a, rtol=0, atol=1e-10 * o.a.max())
+    np.testing.assert_allclose(c2, o.chi2, rtol=1e-9)
     s.close()
 
 
