@@ -711,6 +711,67 @@ def test_index_walk_untraced_end_state(name, W, L):
     s.close()
 
 
+def test_checkpoint_and_resume_through_the_setters():
+    """Checkpoint = sail_get (spectra, running chi^2) + sail_stats (y) + the sweep counter; resume on a NEW handle with
+    sail_init_walkers(mode 1) + sail_set_walkers (y) + sail_set_chi2 + sail_set_sweep.  The resumed run continues the
+    same Philox streams and ends where the uninterrupted run ends (the model is recomputed from the spectra at the
+    resume, so agreement is to rounding, not bit for bit); the device-side and caller-buffer forms of sail_get and the
+    asynchronous branching call give what the host forms give."""
+    import torch
+    w = wl.make("small", simpson_intervals=20_000)
+    W = 150
+    T = wl.geometric_schedule(1.0, 0.2, 8)
+    sa = _sail(w, W)
+    sa.init_walkers(W, w.A, w.B, SEED)
+    sa.anneal(T[:4], w.eta)
+    ck_a, ck_c2 = sa.get()
+    _, _, ck_y = sa.stats()
+    sa.anneal(T[4:], w.eta)
+    a_ref, c2_ref = sa.get()
+    sb = _sail(w, W)
+    sb.init_walkers(W, w.A, w.B, SEED, spectra=ck_a)
+    sb.set_walkers(0, ck_a, y=ck_y)
+    sb.set_chi2(ck_c2)
+    sb.set_sweep(4)
+    sb.anneal(T[4:], w.eta)
+    a_res, c2_res = sb.get()
+    np.testing.assert_allclose(a_res, a_ref, rtol=0, atol=1e-9 * a_ref.max())
+    np.testing.assert_allclose(c2_res, c2_ref, rtol=1e-9, atol=1e-14 * float(ck_c2.max()))
+    np.testing.assert_allclose(sb.stats()[2], sa.stats()[2], rtol=1e-15)           # y: same acceptance counts per sweep
+    # a wrong sweep counter gives other random numbers, hence another end state
+    sc = _sail(w, W)
+    sc.init_walkers(W, w.A, w.B, SEED, spectra=ck_a)
+    sc.set_walkers(0, ck_a, y=ck_y)
+    sc.anneal(T[4:], w.eta)
+    assert np.abs(sc.get()[0] - a_ref).max() > 1e-6 * a_ref.max()
+    # the other forms of sail_get, and sail_branch without outputs
+    sp_t = torch.empty((W, w.n_omega), dtype=torch.float64, device="cuda")
+    c2_t = torch.empty(W, dtype=torch.float64, device="cuda")
+    sa.get_device(sp_t, c2_t)
+    torch.cuda.synchronize()
+    assert np.array_equal(sp_t.cpu().numpy(), a_ref) and np.array_equal(c2_t.cpu().numpy(), c2_ref)
+    sp_h, c2_h = np.empty((W, w.n_omega)), np.empty(W)
+    sa.get_into(sp_h, c2_h)
+    assert np.array_equal(sp_h, a_ref) and np.array_equal(c2_h, c2_ref)
+    # sail_branch with no output requested (stream-ordered): the same event as the call that reads the maps back
+    sb.set_walkers(0, a_ref, y=sa.stats()[2])
+    sb.set_chi2(c2_ref)
+    sb.set_sweep(8)
+    Tb = float(np.std(c2_ref))
+    sa.branch_async(Tb, 0.1)
+    info, mult, donor = sb.branch(Tb, 0.1, want_maps=True)
+    assert info.n_recipients > 0 and mult.sum() == W
+    a_async, a_sync = sa.get()[0], sb.get()[0]
+    keep = mult > 0                                           # walkers that are not recipients: untouched by the event
+    assert np.array_equal(a_async[keep], a_ref[keep]) and np.array_equal(a_sync[keep], a_ref[keep])
+    np.testing.assert_allclose(a_async, a_sync, rtol=0, atol=1e-12 * a_ref.max())
+    wm = w.omega + 0.5 * w.domega
+    np.testing.assert_allclose(a_async.sum(axis=1), w.A, rtol=1e-11)
+    np.testing.assert_allclose((a_async * wm).sum(axis=1), w.B, rtol=1e-11)
+    for h in (sa, sb, sc):
+        h.close()
+
+
 def test_sharded_population_draws_the_single_handle_streams():
     """sail_set_walker_offset: two handles owning walkers [0, 40) and [40, 97) of a population
     make, without branching, exactly the moves of one handle that owns all 97."""
