@@ -294,6 +294,8 @@ def main_ours(args):
     from paper_1609_07936_b200.binding import Sail, measure_fp64_peak
 
     rank, local_rank, world = sdist.init("nccl")
+    if local_rank >= torch.cuda.device_count():
+        raise SystemExit(f"bench.py: rank {rank} needs cuda:{local_rank} but this node has {torch.cuda.device_count()} GPU(s)")
     torch.cuda.set_device(local_rank)
     dev = f"cuda:{local_rank}"
     w = wl.make(args.workload)
@@ -361,6 +363,40 @@ def main_ours(args):
     value = total_moves / total_s
     ms_per_step = 1e3 * total_s / args.steps
 
+    # ---- end to end through the C ABI with host buffers: the same K steps, on every rank ------------------
+    e2e = None
+    if args.e2e:
+        host_sp = torch.empty((w.W, w.n_omega), dtype=torch.float64).pin_memory().numpy()
+        host_c2 = torch.empty(w.W, dtype=torch.float64).pin_memory().numpy()
+        n_e2e = args.steps if args.e2e < 0 else min(args.steps, args.e2e)
+        torch.cuda.synchronize()
+        sdist.barrier(dev)
+        s2 = None
+        t0 = time.perf_counter()
+        for i in range(n_e2e):
+            b = i % nb
+            if b == 0:
+                if s2 is not None:
+                    s2.close()
+                s2 = Sail(w.omega, w.tau, w.F, w.sigma, max_walkers=w.W, device=local_rank)     # H2D of the problem
+                s2.init_walkers(w.W, w.A, w.B, seed)
+            run_block(s2, w, b, torch, host_out=(host_sp, host_c2))    # schedule slice H2D, chi^2 (and spectra) D2H
+        torch.cuda.synchronize()
+        s2.close()
+        dt = time.perf_counter() - t0
+        # every rank runs its replica through host buffers: max time over ranks, units of all ranks (whole-job rate)
+        dt_max, units_all = sdist.reduce_timing(dt, float(step_moves * n_e2e), dev)
+        if n_e2e == args.steps and args.steps % nb == 0:
+            assert np.array_equal(host_c2, chi2_final), "e2e run is not bit-identical to the device-resident run"
+        n_anneals = max(1, (n_e2e + nb - 1) // nb)
+        h2d = 8 * bs + 8 * (w.n_omega + 3 * w.n_tau) * n_anneals / n_e2e
+        d2h = 8 * w.W + 8 * w.W * w.n_omega * (n_e2e // nb) / n_e2e
+        e2e = {"value": units_all / dt_max, "unit": UNIT, "h2d_bytes_per_step": world * h2d, "d2h_bytes_per_step": world * d2h,
+               "steps": n_e2e, "ms_per_step": 1e3 * dt_max / n_e2e,
+               "includes": "sail_create + sail_init_walkers at the first block of an anneal, per block: schedule slice H2D, sweeps, resync, "
+                           "branching, chi^2 of all walkers to pinned host memory; spectra to the host after the last block; sail_destroy"}
+
+
     line = None
     if rank == 0:
         # ---- roofline of the dominant kernel (the sweep kernel): FP64 ALU bound ----------------------
@@ -392,37 +428,8 @@ def main_ours(args):
         except Exception as ex:  # supplementary only
             roofline["credited_loop_alone"] = {"error": repr(ex)}
 
-        # ---- end to end through the C ABI with host buffers: the same K steps --------------------------------
-        e2e = None
-        if args.e2e:
-            host_sp = torch.empty((w.W, w.n_omega), dtype=torch.float64).pin_memory().numpy()
-            host_c2 = torch.empty(w.W, dtype=torch.float64).pin_memory().numpy()
-            n_e2e = args.steps if args.e2e < 0 else min(args.steps, args.e2e)
-            torch.cuda.synchronize()
-            s2 = None
-            t0 = time.perf_counter()
-            for i in range(n_e2e):
-                b = i % nb
-                if b == 0:
-                    if s2 is not None:
-                        s2.close()
-                    s2 = Sail(w.omega, w.tau, w.F, w.sigma, max_walkers=w.W, device=local_rank)     # H2D of the problem
-                    s2.init_walkers(w.W, w.A, w.B, seed)
-                run_block(s2, w, b, torch, host_out=(host_sp, host_c2))    # schedule slice H2D, chi^2 (and spectra) D2H
-            torch.cuda.synchronize()
-            s2.close()
-            dt = time.perf_counter() - t0
-            if n_e2e == args.steps and args.steps % nb == 0:
-                assert np.array_equal(host_c2, chi2_final), "e2e run is not bit-identical to the device-resident run"
-            n_anneals = max(1, (n_e2e + nb - 1) // nb)
-            h2d = 8 * bs + 8 * (w.n_omega + 3 * w.n_tau) * n_anneals / n_e2e
-            d2h = 8 * w.W + 8 * w.W * w.n_omega * (n_e2e // nb) / n_e2e
-            e2e = {"value": step_moves * n_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                   "steps": n_e2e, "ms_per_step": 1e3 * dt / n_e2e,
-                   "includes": "sail_create + sail_init_walkers at the first block of an anneal, per block: schedule slice H2D, sweeps, resync, "
-                               "branching, chi^2 of all walkers to pinned host memory; spectra to the host after the last block; sail_destroy"}
-
-        cpu_v, cores, sample = cpu_oracle_sample(w, target_s=args.cpu_seconds)
+        # the oracle on the host cores: rank 0, N = 1 only
+        cpu_v, cores, sample = cpu_oracle_sample(w, target_s=args.cpu_seconds) if world == 1 else (None, None, None)
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
@@ -436,7 +443,7 @@ def main_ours(args):
                            "attempted_moves_per_step": step_moves, "blocks_per_anneal": nb},
                 "anneals_per_s": world * args.steps / nb / total_s,
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
-                "cpu_baseline": {"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+                "cpu_baseline": ({"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample} if world == 1 else None),
                 "chi2_final_median": float(np.median(chi2_final))}
     s.close()
     del spectra_t, chi2_t, flush
