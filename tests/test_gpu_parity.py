@@ -711,6 +711,50 @@ def test_index_walk_untraced_end_state(name, W, L):
     s.close()
 
 
+_SHAPES = [(2, 1, 1), (3, 33, 33), (4, 32, 3), (64, 64, 65), (31, 96, 2), (255, 128, 5), (257, 129, 7), (33, 512, 3),
+           (600, 31, 9), (1023, 1, 4), (128, 160, 40), (389, 7, 61), (50, 321, 2), (17, 200, 19), (300, 224, 31), (96, 225, 12)]
+
+
+@pytest.mark.parametrize("n_omega,n_tau,W", _SHAPES)
+def test_arbitrary_grid_shapes_end_state_parity(n_omega, n_tau, W):
+    """Grid sizes and populations off the five configurations (two bins, one tau-point, N_tau at and next to multiples of
+    32, ragged W, every C of the kernel): the untraced path — sweeps with and without the index walk across a resync
+    boundary, then one branching event — against the oracle.  The absolute chi^2 term is reading T3 of DESIGN.md section 7
+    (with a single tau-point the residue is zero up to rounding on both sides, Eq. 16)."""
+    k = _SHAPES.index((n_omega, n_tau, W))
+    L = k % 3 if n_omega > 2 else 0
+    w = wl.random_problem(100 + k, n_omega, n_tau, omega_max=(4.0, 6.0, 10.0)[k % 3], dtau=(0.02, 0.07, 0.2)[(k // 3) % 3],
+                          eps=(1e-2, 1e-3, 1e-4)[k % 3])
+    eta = min(w.eta, 0.4)                                        # 4 / N_omega is not < 1 on a handful of bins
+    T = wl.geometric_schedule(1.0, 0.2, 4)
+    o = oracle.Oracle(w.omega, w.tau, w.F, w.sigma, w.A, w.B, eta, SEED, walk_len=L)
+    o.init_walkers(W)
+    chi2_0 = float(np.abs(o.chi2).max())
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED, spectra=o.a)
+    assert s.anneal(T, eta, resync_every=3, walk_length=L) == (None, None)
+    o.anneal(T, resync_every=3)
+    a, c2 = s.get()
+    acc, ev, y = s.stats()
+    np.testing.assert_array_equal(acc, o.acc)
+    np.testing.assert_array_equal(ev, o.feas)
+    np.testing.assert_allclose(y, o.y, rtol=1e-15, atol=0)
+    np.testing.assert_allclose(a, o.a, rtol=0, atol=1e-10 * o.a.max())
+    # absolute terms: the running-sum history (T3) and the rounding floor of a residual that is zero by construction
+    # (one tau-point: Eq. 16 makes M_0 = F_0 exactly): (eps F / sigma)^2 ~ 1e-32 sum (F / sigma)^2
+    floor = 1e-24 * float(((w.F / w.sigma) ** 2).sum())
+    np.testing.assert_allclose(c2, o.chi2, rtol=1e-9, atol=1e-14 * chi2_0 + floor)
+    if W > 1:
+        s.set_walkers(0, o.a, y=o.y)
+        s.set_chi2(o.chi2)
+        Tb = float(np.std(o.chi2)) or 1.0
+        info, mult, donor = s.branch(Tb, 0.3, want_maps=True)
+        n_rec, mo, do = o.branch(Tb, 0.3)
+        assert (mult == mo).all() and (donor == do).all() and info.n_recipients == n_rec
+        np.testing.assert_allclose(s.get()[0], o.a, rtol=0, atol=1e-12 * o.a.max())
+    s.close()
+
+
 def test_checkpoint_and_resume_through_the_setters():
     """Checkpoint = sail_get (spectra, running chi^2) + sail_stats (y) + the sweep counter; resume on a NEW handle with
     sail_init_walkers(mode 1) + sail_set_walkers (y) + sail_set_chi2 + sail_set_sweep.  The resumed run continues the
