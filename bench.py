@@ -44,11 +44,11 @@ DFMA_PER_TAU_POINT = 5          # algorithmic FP64-pipe instructions per tau-poi
 NAMES = ["tiny", "small", "branching", "noise", "stress"]
 
 # dram__bytes_read.sum + dram__bytes_write.sum of ONE sweep-kernel launch, from the committed `ncu --set full` captures
-# profiles/r02_sweep_{stress,noise,small}_full_metrics.txt (2-sweep launches).  A warp runs ALL sweeps of a launch on a
+# profiles/r02_sweep_{stress,noise,branching,small,tiny}_full_metrics.txt (2-sweep launches).  A warp runs ALL sweeps of a launch on a
 # walker while that walker's spectrum and model are resident on chip, so the DRAM traffic of a launch is the walker state
 # once in and once out (algorithmic: 16 W (N_omega + N_tau) bytes) whatever the number of sweeps; states that fit the
 # 126 MB L2 (small, noise) partly stay there between launches.
-SWEEP_DRAM_BYTES_PER_LAUNCH = {"stress": 11.094e9, "noise": 0.2822e9, "small": 11.9e6}
+SWEEP_DRAM_BYTES_PER_LAUNCH = {"stress": 11.094e9, "noise": 0.2822e9, "branching": 0.6969e9, "small": 11.9e6, "tiny": 92.4e3}
 
 
 # ------------------------------------------------------------------------------------------------
