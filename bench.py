@@ -190,6 +190,15 @@ def main_reference(args):
         return 0
     w = wl.make(args.workload)
     bs, nb = block_layout(w)
+    if args.cpu_whole:
+        # the oracle on the WHOLE anneal of the workload, once (BASELINE.md asks for it on Tiny and Small; Small takes minutes)
+        v, cores, sample = cpu_oracle_sample(w, whole=True)
+        print(json.dumps({"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": 1, "warmup": 0,
+                          "ms_per_step": 1e3 * w.attempted_moves() / v, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                          "dtype": "f64", "data": "synthetic", "config": {"workload": workload_string(w), "step": "one whole anneal on the CPU oracle"},
+                          "cpu_baseline": {"value": v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+                          "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+        return 0
     vals = []
     for _ in range(args.warmup):
         cpu_oracle_sample(w, target_s=1.0)
@@ -607,6 +616,7 @@ if __name__ == "__main__":
     ap.add_argument("--workload", default="stress", choices=NAMES)
     ap.add_argument("--sweeps", type=int, default=0, help="override the number of sweeps (debug)")
     ap.add_argument("--cpu-seconds", type=float, default=12.0)
+    ap.add_argument("--cpu-whole", action="store_true", help="--impl reference: time the oracle on the whole anneal of the workload, once")
     ap.add_argument("--e2e", type=int, default=-1, help="steps of the end-to-end (host buffers) run; -1 = as many as --steps, 0 = skip")
     ap.add_argument("--configs", type=int, default=1, help="also run one whole anneal of each BASELINE.json configuration (N=1 only)")
     ap.add_argument("--extra", type=int, default=1, help="also time resync / smoothing / branching / walk rows and the microbenchmarks (N=1 only)")
