@@ -188,6 +188,43 @@ SAIL_API int sail_smooth(sail_t *h, double s);
  */
 SAIL_API int sail_chi2_stats(sail_t *h, double *chi2_min, double *chi2_mean);
 
+/*
+ * sail_chi2_stats_static — the same two statistics (smallest and mean residue) for callers that must
+ * not allocate device memory and have no handle whose workspace they could borrow.
+ *
+ * Who that is.  A handle belongs to one thread at a time, so a second thread that watches an anneal in progress (a
+ * progress monitor, a stopping rule, a logger on its own stream) works on a COPY of the residues — e.g. the tensor it
+ * got from sail_get(..., on_device = 1) — and cannot touch the handle or its workspace.  That thread cannot call
+ * cudaMalloc / cudaFree either: both wait for the whole device, and a sweep-kernel launch of the large configurations
+ * runs for seconds, so one such call stalls the monitor for that long (and cudaFree stalls the anneal's stream too).
+ * The same holds for a process in which a framework's caching allocator (torch's) already owns all of HBM: a raw
+ * cudaMalloc from this library then fails although the framework still has free blocks.
+ *
+ * What it does instead.  The per-CTA partial sums and minima go to a fixed array that is part of the library image
+ * (a file-scope __device__ array of SAIL_STATS_STATIC_SCRATCH_BYTES = 4096 bytes; every GPU that loads the library
+ * holds these 4 KB until the process exits).  No cudaMalloc, cudaFree or allocating library routine is called.
+ *
+ *   device  CUDA device ordinal (made current);  stream  cudaStream_t to enqueue on, NULL = default stream
+ *   chi2    DEVICE [W] residues, read only;  1 <= W <= SAIL_STATS_STATIC_MAX_W (2^24).  The array holds 256 partial
+ *           results whatever W is; the bound is the population size up to which a thread adds at most 256 residues one
+ *           after the other, i.e. up to which the mean is good to ~600 eps relative for residues of one sign.  Larger
+ *           W: SAIL_ERR_ARG with the limit in the error text — use sail_chi2_stats (handle workspace) or split the array.
+ *   out     DEVICE [2], written stream-ordered: out[0] = min, out[1] = mean.  Same kernels, same summation order and
+ *           so the same bits as sail_chi2_stats on the same residues.  The call does not synchronise.
+ *
+ * Set-up.  The first call on each device looks up the device address of the array (cudaGetSymbolAddress with that device
+ * current; an error is returned as SAIL_ERR_CUDA).  Make that first call during start-up, outside any stream capture;
+ * later calls only enqueue two kernels.
+ * Sharing.  There is ONE array per device, shared by every call from every thread, and it keeps what the last call
+ * left in it.  Nothing in it has to start at zero (each call overwrites every slot it later reads), so two calls in a
+ * row need no clearing — but two calls whose kernels can run at the same time on one GPU (different streams, no event
+ * between them) race on it and return garbage.  Keep the calls of one device on one stream, or order them with events.
+ * Errors go to sail_last_error(NULL) of the calling thread.
+ */
+#define SAIL_STATS_STATIC_MAX_W ((int64_t)1 << 24)
+#define SAIL_STATS_STATIC_SCRATCH_BYTES 4096
+SAIL_API int sail_chi2_stats_static(int32_t device, void *stream, const double *chi2, int64_t W, double *out);
+
 /* Parameters of sail_anneal_selfcool (readings C1-C3; the paper gives no constants beyond T_start). */
 typedef struct {
     int32_t sweeps_per_block;   /* k of "each block consists of some k N_omega steps" (paper: 100, :218)          */

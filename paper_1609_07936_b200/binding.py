@@ -18,7 +18,8 @@ SAIL_OK, SAIL_ERR_ARG, SAIL_ERR_GRID, SAIL_ERR_ALLOC, SAIL_ERR_CUDA, SAIL_ERR_ST
 
 EXPORTS = ["sail_workspace_bytes", "sail_create", "sail_init_walkers", "sail_anneal", "sail_branch",
            "sail_resync", "sail_get", "sail_get_model", "sail_stats", "sail_set_walkers", "sail_set_sweep",
-           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak", "sail_microbench", "sail_smooth", "sail_chi2_stats", "sail_anneal_selfcool", "sail_branch_fraction", "sail_set_walker_offset", "sail_set_chi2"]
+           "sail_destroy", "sail_last_error", "sail_launch_count", "sail_measure_fp64_peak", "sail_microbench", "sail_smooth", "sail_chi2_stats", "sail_anneal_selfcool", "sail_branch_fraction", "sail_set_walker_offset", "sail_set_chi2",
+           "sail_chi2_stats_static"]
 
 
 class SailError(RuntimeError):
@@ -79,6 +80,7 @@ def lib():
         L.sail_branch_fraction.argtypes = [C.c_void_p, C.c_double, C.c_double, C.POINTER(C.c_double),
                                            C.POINTER(sail_branch_info), C.c_void_p, C.c_void_p]
         L.sail_chi2_stats.argtypes = [C.c_void_p, C.POINTER(C.c_double), C.POINTER(C.c_double)]
+        L.sail_chi2_stats_static.argtypes = [C.c_int32, C.c_void_p, C.c_void_p, C.c_int64, C.c_void_p]
         L.sail_anneal_selfcool.argtypes = [C.c_void_p, C.POINTER(sail_selfcool_params), C.c_int64, C.c_void_p,
                                            C.c_void_p, C.c_void_p]
         L.sail_get.argtypes = [C.c_void_p, C.c_void_p, C.c_void_p, C.c_int32]
@@ -132,6 +134,31 @@ def microbench(device=0):
     if rc:
         raise SailError(rc, lib().sail_last_error(None).decode())
     return {k: float(v) for k, v in zip(MICROBENCH_KEYS, out)}
+
+
+STATS_STATIC_MAX_W = 1 << 24     # include/sail.h: SAIL_STATS_STATIC_MAX_W
+
+
+def chi2_stats_static(chi2_t, out_t, n=None):
+    """(min, mean) of the residues in the CUDA float64 tensor `chi2_t` (first `n` entries; default all) into the
+    CUDA float64 tensor `out_t` (2 entries), enqueued on torch's current stream of that device, without a handle and
+    without any device allocation: for a thread that watches an anneal from a copy of the residues and can neither
+    use the handle (one thread at a time) nor afford cudaMalloc's device-wide wait.  The scratch is one fixed 4 KB
+    array per GPU shared by all calls: keep the calls of a device on one stream (include/sail.h:
+    sail_chi2_stats_static).  Nothing is copied or synchronised here; read `out_t` when you need the numbers."""
+    import torch
+    if not (chi2_t.is_cuda and out_t.is_cuda and chi2_t.dtype == torch.float64 and out_t.dtype == torch.float64
+            and chi2_t.is_contiguous() and out_t.is_contiguous() and out_t.numel() >= 2
+            and chi2_t.device == out_t.device):
+        raise ValueError("chi2_t and out_t must be contiguous float64 CUDA tensors on one device, out_t with >= 2 entries")
+    n = chi2_t.numel() if n is None else int(n)
+    if n > chi2_t.numel():
+        raise ValueError("n exceeds the tensor")
+    dev = chi2_t.device.index
+    rc = lib().sail_chi2_stats_static(dev, C.c_void_p(torch.cuda.current_stream(dev).cuda_stream),
+                                      C.c_void_p(chi2_t.data_ptr()), n, C.c_void_p(out_t.data_ptr()))
+    if rc:
+        raise SailError(rc, lib().sail_last_error(None).decode())
 
 
 class Sail:

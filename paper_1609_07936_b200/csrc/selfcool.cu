@@ -7,6 +7,8 @@
 // run to run), the rule (one thread), the block's schedule slice, the acceptance-driven strength (reading B7) and the
 // parameters of the branching event live in the handle's control block; the host only enqueues.  T / chi2_ave /
 // chi2_min per block come back once at the end of the call.
+#include <mutex>
+
 #include "sail_internal.cuh"
 
 namespace sail {
@@ -202,3 +204,79 @@ int sail_anneal_selfcool(sail_t *h, const sail_selfcool_params *p, int64_t n_blo
 }
 
 } // extern "C"
+
+// ---------------------------------------------------------------------------------------------------------------------
+// sail_chi2_stats_static — the population statistics for callers that may not allocate (include/sail.h says who: a
+// monitoring thread without the handle, or a process whose HBM a caching allocator already owns).  The two kernels above
+// are reused unchanged; only the place their per-CTA partial results go differs: a fixed array in the library image
+// instead of a slice of a handle's workspace.
+// ---------------------------------------------------------------------------------------------------------------------
+namespace sail {
+
+// kStatBlocks partial sums followed by kStatBlocks partial minima = SAIL_STATS_STATIC_SCRATCH_BYTES.  One copy per GPU
+// that loads the library, alive until the process exits, shared by every call on that GPU.
+static __device__ __align__(256) double g_stats_static_scratch[2 * kStatBlocks];
+static_assert(sizeof(double) * 2 * kStatBlocks == SAIL_STATS_STATIC_SCRATCH_BYTES, "sail.h states the size of the static scratch array");
+static_assert(SAIL_STATS_STATIC_MAX_W == (int64_t)kStatBlocks * kStatThreads * 256, "sail.h: at most 256 residues per thread");
+
+// In host code the name g_stats_static_scratch is only a stand-in for the symbol, NOT a device address: a kernel handed
+// `g_stats_static_scratch` from the host faults (or scribbles over host memory where the GPU can reach it).  The device
+// address differs from GPU to GPU and is looked up once per device with cudaGetSymbolAddress, with that device current.
+constexpr int kStaticMaxDevices = 64;
+static std::mutex g_stats_static_mutex;
+static double *g_stats_static_addr[kStaticMaxDevices];      // nullptr = this device has not been set up yet
+
+// `device` must be current.  Allocates nothing: the array already exists in the module loaded on the device.
+static int stats_static_scratch(int device, double **scratch)
+{
+    std::lock_guard<std::mutex> lock(g_stats_static_mutex);
+    if (!g_stats_static_addr[device]) {
+        void *p = nullptr;
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_stats_static_scratch);
+        if (e != cudaSuccess || !p) {
+            cudaGetLastError();
+            return set_err(nullptr, SAIL_ERR_CUDA, "sail_chi2_stats_static: cudaGetSymbolAddress on device %d failed: %s", device,
+                           cudaGetErrorString(e));
+        }
+        g_stats_static_addr[device] = static_cast<double *>(p);
+    }
+    *scratch = g_stats_static_addr[device];
+    return SAIL_OK;
+}
+
+} // namespace sail
+
+extern "C" int sail_chi2_stats_static(int32_t device, void *stream, const double *chi2, int64_t W, double *out)
+{
+    using namespace sail;
+    if (!chi2 || !out) return set_err(nullptr, SAIL_ERR_ARG, "sail_chi2_stats_static: chi2 and out must be device pointers, not NULL");
+    if (W < 1 || W > SAIL_STATS_STATIC_MAX_W)
+        return set_err(nullptr, SAIL_ERR_ARG, "sail_chi2_stats_static: W=%lld outside [1, %lld] (SAIL_STATS_STATIC_MAX_W: the fixed %d-byte "
+                       "scratch array is laid out for at most that many residues; use sail_chi2_stats or split the array)",
+                       (long long)W, (long long)SAIL_STATS_STATIC_MAX_W, SAIL_STATS_STATIC_SCRATCH_BYTES);
+    int ndev = 0;
+    if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1 || device < 0 || device >= ndev) {
+        cudaGetLastError();
+        return set_err(nullptr, SAIL_ERR_CUDA, "sail_chi2_stats_static: no usable CUDA device (count=%d, requested=%d); there is no CPU fallback", ndev, device);
+    }
+    if (device >= kStaticMaxDevices) return set_err(nullptr, SAIL_ERR_ARG, "sail_chi2_stats_static: device ordinal %d >= %d", device, kStaticMaxDevices);
+    if (cudaSetDevice(device) != cudaSuccess) { cudaGetLastError(); return set_err(nullptr, SAIL_ERR_CUDA, "sail_chi2_stats_static: cudaSetDevice(%d) failed", device); }
+    double *scratch = nullptr;
+    if (const int rc = stats_static_scratch(device, &scratch)) return rc;
+    // the grid of enqueue_chi2_stats, so that the summation order (and with it every bit of the result) is the same
+    int blocks = (int)((W + kStatThreads - 1) / kStatThreads);
+    if (blocks > kStatBlocks) blocks = kStatBlocks;
+    if (blocks > W / 2) blocks = (int)(W / 2 > 0 ? W / 2 : 1);
+    double *partial = scratch, *pmin = scratch + kStatBlocks;
+    // Nothing to clear: the first kernel writes slots [0, blocks) of both halves, the second reads exactly those, so what an
+    // earlier call (possibly with more CTAs) left behind is never read.
+    cudaStream_t st = (cudaStream_t)stream;
+    chi2_stats_partial_kernel<<<blocks, kStatThreads, 0, st>>>((long long)W, chi2, partial, pmin);
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess) {
+        chi2_stats_final_kernel<<<1, 1, 0, st>>>(blocks, (long long)W, partial, pmin, out);
+        e = cudaGetLastError();
+    }
+    if (e != cudaSuccess) return set_err(nullptr, SAIL_ERR_CUDA, "sail_chi2_stats_static: kernel launch failed: %s", cudaGetErrorString(e));
+    return SAIL_OK;
+}
