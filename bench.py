@@ -51,6 +51,24 @@ NAMES = ["tiny", "small", "branching", "noise", "stress"]
 SWEEP_DRAM_BYTES_PER_LAUNCH = {"stress": 11.094e9, "noise": 0.2822e9, "branching": 0.6969e9, "small": 11.9e6, "tiny": 92.4e3}
 
 
+# Whole-anneal sweep-kernel fractions of the NOMINAL FP64 rate in the driver-run lines of the earlier rounds
+# (profiles/r01_all_configs.md, profiles/r02_bench_stress.json.txt `configs`), so that a change of the headline workload
+# is not read as kernel progress: the headline was Small in round 1 and is Stress since round 2.  This round's figures
+# are `configs[*].roofline_frac` of the same line (also of the nominal rate).
+HISTORY = {"headline_workload": {"r01": "small", "r02": "stress", "r03": "stress"},
+           "sweep_kernel_frac_of_nominal": {"r01": {"tiny": 0.002, "small": 0.177, "branching": 0.280, "noise": 0.305, "stress": 0.395},
+                                            "r02": {"tiny": 0.002, "small": 0.173, "branching": 0.278, "noise": 0.305, "stress": 0.398}},
+           "note": "r01 -> r02 changed no configuration by more than 0.004: the round-2 headline gain (0.176 -> 0.398) is the workload switch"}
+
+
+def build_defines():
+    """The -D flags the library on disk was built with (paper_1609_07936_b200/build/defines.txt); [] = the product library."""
+    try:
+        return open(os.path.join(ROOT, "paper_1609_07936_b200", "build", "defines.txt")).read().split()
+    except OSError:
+        return None
+
+
 # ------------------------------------------------------------------------------------------------
 class ClockSampler:
     """Samples nvidia-smi clocks / throttle reasons during the timed region."""
@@ -155,6 +173,26 @@ def run_block(s, w, b, torch, dev_out=None, host_out=None):
     return e0, e1
 
 
+def l2_is_flushed(w):
+    """Small walker states would sit in the 126 MB L2 between steps: they are flushed (256 MiB write) between steps."""
+    return 8 * w.W * (w.n_omega + w.n_tau) < 512 * 1024 * 1024
+
+
+def config_dict(w, world):
+    """The `config` object of the JSON line: one definition for our arm and for the reference arm (--impl reference),
+    so that both name the same workload and the same step."""
+    bs, nb = block_layout(w)
+    state_bytes = 8 * w.W * (w.n_omega + w.n_tau)
+    return {"workload": workload_string(w),
+            "step": (f"one protocol block: {bs} sweeps (+ resync / imprinted branching as configured); {nb} blocks = one whole anneal; "
+                     "walkers re-initialised untimed when the block index wraps") if nb > 1 else
+                    "one whole anneal (all sweeps + final sail_get), walkers re-initialised untimed",
+            "parallelism": f"{world} independent replica(s), one per GPU",
+            "l2": "flushed between steps (256 MiB write)" if l2_is_flushed(w) else
+                  f"not flushed: the walker state a step streams ({state_bytes / 2**30:.1f} GiB) is larger than L2 (126 MB)",
+            "attempted_moves_per_step": w.W * bs * w.n_omega, "blocks_per_anneal": nb}
+
+
 def cpu_oracle_sample(w, target_s=12.0, seed=0x5A11, whole=False):
     """Oracle (as it stands) on the host cores.  whole = False: a bounded sample (a subset of walkers over the first
     sweeps of the schedule); whole = True: the whole anneal of the workload (Tiny / Small only).
@@ -211,10 +249,10 @@ def main_reference(args):
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * step_moves / value,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": workload_string(w),
-                       "step": "a bounded sample of the workload per step (CPU oracle on the host cores); ms_per_step = one "
-                               "protocol block of the workload at the measured rate (extrapolated)"},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "config": config_dict(w, max(args.gpus, 1)),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": sample + f"; one such bounded sample per step, {args.steps} steps, value = their mean; ms_per_step = the "
+                                                "time of one step of `config` (a protocol block) at that rate, extrapolated, not run"},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line))
@@ -226,7 +264,7 @@ def main_selfcool(args):
     branched with t = 0.1, strength following the acceptance rate) on the chosen workload; prints the trajectory."""
     import torch
     from paper_1609_07936_b200 import build
-    build.build()
+    build.build(defines=None if args.diag_defines else ())
     from paper_1609_07936_b200.binding import Sail
     w = wl.make(args.workload)
     s = Sail(w.omega, w.tau, w.F, w.sigma, max_walkers=w.W)
@@ -299,7 +337,7 @@ def main_ours(args):
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the oracle")
     from paper_1609_07936_b200 import build
-    build.build()
+    build.build(defines=None if args.diag_defines else ())
     from paper_1609_07936_b200.binding import Sail, measure_fp64_peak
 
     rank, local_rank, world = sdist.init("nccl")
@@ -314,7 +352,7 @@ def main_ours(args):
     seed = sdist.rank_seed(w.rng_seed, rank)          # every rank anneals an independent replica (weak scaling)
     peaks = measured_peaks()
     state_bytes = 8 * w.W * (w.n_omega + w.n_tau)
-    l2_flush = state_bytes < 512 * 1024 * 1024        # small states would sit in the 126 MB L2 between steps
+    l2_flush = l2_is_flushed(w)
 
     spectra_t = torch.empty((w.W, w.n_omega), dtype=torch.float64, device=dev)
     chi2_t = torch.empty(w.W, dtype=torch.float64, device=dev)
@@ -416,11 +454,17 @@ def main_ours(args):
         kern_total = float(np.sum(kern_s))
         achieved = DFMA_PER_TAU_POINT * w.n_tau * evaluated / kern_total
         attempted = float(step_moves * args.steps)
-        roofline = {"bound": "alu", "kernel": "sail::sweep_kernel", "achieved": achieved / 1e12, "peak": peak_nominal / 1e12,
-                    "unit": "T FP64 lane-instr/s", "frac": achieved / peak_nominal,
+        # the denominator is the DFMA rate MEASURED in this run (register-resident two-operand DFMA chains,
+        # sail_measure_fp64_peak); the nominal rate (unit count x clock) is kept beside it
+        roofline = {"bound": "alu", "kernel": "sail::sweep_kernel", "achieved": achieved / 1e12, "peak": dfma_measured / 1e12,
+                    "unit": "T FP64 lane-instr/s", "frac": achieved / dfma_measured,
                     "traffic": SWEEP_DRAM_BYTES_PER_LAUNCH.get(w.name),
-                    "peak_source": f"derived: {num_sms} SMs x {FP64_LANES_PER_SM} FP64 lanes x {sm_max:.0f} MHz (DESIGN.md §6.1); not in MEASURED_PEAKS.json",
-                    "peak_measured_dfma": dfma_measured / 1e12, "frac_of_measured_dfma": achieved / dfma_measured,
+                    "traffic_source": (f"not from this run: dram__bytes_read.sum + dram__bytes_write.sum of one sweep-kernel launch in the committed "
+                                       f"`ncu --set full` capture profiles/r02_sweep_{w.name}_full_metrics.txt (a 2-sweep launch; the traffic of a launch "
+                                       "is the walker state once in and once out whatever its number of sweeps)"),
+                    "peak_source": "measured in this run: sail_measure_fp64_peak, register-resident DFMA chains (FP64 is not in MEASURED_PEAKS.json)",
+                    "peak_nominal": peak_nominal / 1e12, "frac_of_nominal": achieved / peak_nominal,
+                    "peak_nominal_source": f"derived: {num_sms} SMs x {FP64_LANES_PER_SM} FP64 lanes x {sm_max:.0f} MHz (DESIGN.md §6.1)",
                     "algorithmic_instr_per_launch": DFMA_PER_TAU_POINT * w.n_tau * evaluated / max(args.steps, 1),
                     "launch_ms": 1e3 * kern_total / max(args.steps, 1),
                     "evaluated_moves_per_s": evaluated / kern_total,
@@ -442,18 +486,13 @@ def main_ours(args):
         line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
                 "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                 "dtype": "f64", "data": "synthetic",
-                "config": {"workload": workload_string(w),
-                           "step": (f"one protocol block: {bs} sweeps (+ resync / imprinted branching as configured); {nb} blocks = one whole anneal; "
-                                    "walkers re-initialised untimed when the block index wraps") if nb > 1 else
-                                   "one whole anneal (all sweeps + final sail_get), walkers re-initialised untimed",
-                           "parallelism": f"{world} independent replica(s), one per GPU",
-                           "l2": "flushed between steps (256 MiB write)" if l2_flush else
-                                 f"not flushed: the walker state a step streams ({state_bytes / 2**30:.1f} GiB) is larger than L2 (126 MB)",
-                           "attempted_moves_per_step": step_moves, "blocks_per_anneal": nb},
+                "config": config_dict(w, world),
                 "anneals_per_s": world * args.steps / nb / total_s,
                 "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
                 "cpu_baseline": ({"value": cpu_v, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample} if world == 1 else None),
-                "chi2_final_median": float(np.median(chi2_final))}
+                "chi2_final_median": float(np.median(chi2_final)),
+                "build_defines": build_defines(),
+                "history": HISTORY}
     s.close()
     del spectra_t, chi2_t, flush
     if rank == 0:
@@ -465,7 +504,7 @@ def main_ours(args):
                     cfgs[name] = {"workload": workload_string(w), "seconds_per_anneal": total_s * nb / args.steps,
                                   "anneals_per_s": args.steps / nb / total_s, "value": value, "unit": UNIT,
                                   "evaluated_fraction": roofline["evaluated_fraction"], "accepted_fraction": roofline["accepted_fraction"],
-                                  "roofline_frac": roofline["frac"], "clocks": clocks, "note": "the headline run above"}
+                                  "roofline_frac": roofline["frac_of_nominal"], "clocks": clocks, "note": "the headline run above"}
                     continue
                 wc = wl.make(name)
                 entry = whole_anneal(torch, Sail, wc, local_rank, peak_nominal, wc.rng_seed)
@@ -493,7 +532,7 @@ def main_noise_sweep(args):
     anneals each (Philox keys rng_seed + i), W = 16384.  Prints measured anneals/s (no extrapolation)."""
     import torch
     from paper_1609_07936_b200 import build
-    build.build()
+    build.build(defines=None if args.diag_defines else ())
     from paper_1609_07936_b200.binding import Sail
     peaks = measured_peaks()
     peak = torch.cuda.get_device_properties(0).multi_processor_count * FP64_LANES_PER_SM * (peaks.get("sm_max_mhz") or 1965.0) * 1e6
@@ -625,6 +664,9 @@ if __name__ == "__main__":
     ap.add_argument("--selfcool", type=int, default=0, help="run N blocks of the paper's self-cooling protocol instead of the bench (supplementary)")
     ap.add_argument("--noise-sweep", action="store_true", help="run BASELINE.json configs[3] as configured (4 eps x --noise-reps anneals)")
     ap.add_argument("--noise-reps", type=int, default=8)
+    ap.add_argument("--diag-defines", action="store_true",
+                    help="time the library as it is on disk, with whatever -D flags it was built with (python -m paper_1609_07936_b200.build "
+                         "--define ...); default: rebuild the product library (no defines) first.  The flags in force are in `build_defines`")
     a = ap.parse_args()
     if a.noise_sweep:
         sys.exit(main_noise_sweep(a))

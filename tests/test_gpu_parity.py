@@ -16,6 +16,14 @@ pytestmark = pytest.mark.gpu
 SEED = 0x5A11_0000_0000_0001
 
 
+@pytest.fixture(scope="module", autouse=True)
+def _product_library():
+    """The parity tests judge the PRODUCT library: rebuild it without -D flags if a diagnostic build
+    (python -m paper_1609_07936_b200.build --define ...) was left on disk."""
+    from paper_1609_07936_b200 import build
+    build.build(defines=())
+
+
 def _sail(w, W):
     from paper_1609_07936_b200.binding import Sail
     return Sail(w.omega, w.tau, w.F, w.sigma, max_walkers=W)
