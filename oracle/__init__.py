@@ -87,6 +87,14 @@ def selfcool_temperature(b, chi2_0, chi2_ave, chi2_min, n_boil, n_ramp, T_start=
     return chi2_min / (1.0 + freeze_rate * (b - n_boil - n_ramp))
 
 
+def branching_strength_scale(rate, rate_max):
+    """Reading B7 of PAPER.md:184 ("reducing the imprinting strength and the branching fraction according to the
+    decrease of the acceptance probability"): the factor both are multiplied by is the block's acceptance rate
+    relative to the largest block acceptance rate seen so far (which includes this block's).  0 when nothing has been
+    accepted yet."""
+    return rate / rate_max if rate_max > 0.0 else 0.0
+
+
 def stencil(a, s):
     """Eq. 27-29 on one spectrum (no renormalisation)."""
     a = _f64(a)
@@ -217,7 +225,7 @@ class Oracle:
                 rate = (acc_now - acc_prev) / (float(self.W) * float(sweeps_per_block) * float(self.P.n_omega))
                 acc_prev = acc_now
                 acc_max = max(acc_max, rate)
-                scale = rate / acc_max if acc_max > 0.0 else 0.0
+                scale = branching_strength_scale(rate, acc_max)
             if branch_fraction > 0.0:
                 self.branch_fraction(branch_fraction * scale, t_imprint * scale)
             else:

@@ -526,6 +526,102 @@ def test_smooth_restores_both_sum_rules_keeps_positivity_and_resyncs(tiny):
     np.testing.assert_allclose(o2.a, a0, rtol=1e-12)
 
 
+def test_smooth_clamps_the_tilt_where_it_would_turn_a_coefficient_negative(tiny):
+    """Reading S2, positivity branch (PAPER.md:197 "requires an additional renormalization"; Eq. 10, :97, needs
+    a_k >= 0).  Weight piled on the last three bins and s = 0.5: the stencil pushes B down by s domega a_{N-1} (:197), the
+    variance of such a row is a few domega^2, so the tilt that would restore B has 1 + kappa (w_0 - wbar) < 0 — it would
+    make the coefficients of the lowest bins negative.  What the clamp must give, whatever its formula: no negative
+    coefficient; the factor 0 (to one rounding, never below) at the end bin it clamps on — kappa is the largest admissible one; sum a
+    untouched (a tilt about the mean keeps it for ANY kappa); B moved TOWARDS its target, not away and not past it."""
+    n = tiny.n_omega
+    wm = tiny.omega + 0.5 * tiny.domega
+    rng = np.random.Generator(np.random.Philox(5))
+    for row in range(6):
+        a = 1e-3 + rng.uniform(0.0, 1e-3, n)
+        a[-3:] += rng.uniform(5.0, 10.0, 3)
+        A, B = a.sum(), (a * wm).sum()
+        o = oracle.Oracle(tiny.omega, tiny.tau, tiny.F, tiny.sigma, A, B, tiny.eta, 1)
+        o.init_walkers(1, a[None, :].copy())
+        st = oracle.stencil(a, 0.5)
+        B_st = (st * wm).sum()
+        np.testing.assert_allclose(B_st - B, 0.5 * tiny.domega * (a[0] - a[-1]), rtol=1e-9)     # :197, B fell
+        wbar = B_st / A
+        V = (st * (wm - wbar) ** 2).sum()
+        assert 1.0 + (B - B_st) / V * (wm[0] - wbar) < -0.05                                    # the unclamped tilt is inadmissible
+        o.smooth(0.5)
+        out = o.a[0]
+        assert (out >= 0.0).all()
+        # clamped at bin 0: the factor there is 1 + fl(-1/d) d = 0 up to the one rounding of the quotient, from above
+        assert 0.0 <= out[0] <= 2.0 ** -52 * st[0] and st[0] > 0.0 and (out[1:] > 0.0).all()
+        assert abs(out.sum() - A) <= 1e-14 * A
+        B_out = (out * wm).sum()
+        assert B_st < B_out < B and (B - B_out) < (B - B_st)                                    # towards B, not past it
+        # the factor out_k / st_k is linear in w_k through (w_0, 0) and (wbar, 1)
+        np.testing.assert_allclose(out / st, (wm - wm[0]) / (wbar - wm[0]), rtol=0, atol=1e-12)
+        np.testing.assert_array_equal(o.M[0], oracle.forward(o.K, out))                         # resynced
+    # the mirror image (weight on the first bins): the clamp acts at the last bin
+    a = 1e-3 + rng.uniform(0.0, 1e-3, n)
+    a[:3] += rng.uniform(5.0, 10.0, 3)
+    A, B = a.sum(), (a * wm).sum()
+    o = oracle.Oracle(tiny.omega, tiny.tau, tiny.F, tiny.sigma, A, B, tiny.eta, 1)
+    o.init_walkers(1, a[None, :].copy())
+    st = oracle.stencil(a, 0.5)
+    o.smooth(0.5)
+    out = o.a[0]
+    B_st, B_out = (st * wm).sum(), (out * wm).sum()
+    assert (out >= 0.0).all() and out[-1] <= 2.0 ** -52 * st[-1] and abs(out.sum() - A) <= 1e-14 * A
+    assert B < B_out < B_st
+
+
+def test_adaptive_branching_strength_follows_the_acceptance_rate(tiny):
+    """Reading B7 (imprinting strength and branching fraction are reduced "according to the decrease of
+    the acceptance probability").  What the sentence fixes: full strength while the acceptance has not decreased (the
+    block with the largest rate so far), never more than full strength, less when the block's rate is lower, none when
+    nothing is accepted.  Then the protocol: a hot block followed by a cold one — the first branches at full strength
+    (same state as the run without adaptation), the second with strength and fraction both cut by the ratio of the two
+    acceptance rates, so fewer walkers are replaced than without adaptation."""
+    f = oracle.branching_strength_scale
+    rates = [0.40, 0.42, 0.30, 0.35, 0.05, 0.0]
+    best, scales = 0.0, []
+    for r in rates:
+        best = max(best, r)
+        scales.append(f(r, best))
+    assert scales[0] == 1.0 and scales[1] == 1.0                      # at the running maximum
+    assert all(0.0 <= x <= 1.0 for x in scales)
+    assert scales[2] < 1.0 and scales[2] < scales[3] < 1.0 and scales[4] < scales[2] and scales[5] == 0.0
+    np.testing.assert_allclose(scales[2:5], np.array(rates[2:5]) / 0.42, rtol=1e-15)
+    assert f(0.0, 0.0) == 0.0                                         # nothing accepted yet: no branching at all
+
+    W, k, frac, t = 200, 3, 0.25, 0.5
+    hot, cold = 10.0, 1e-9                                            # in units of the starting residue (T_override is absolute)
+    o = _oracle_for(tiny); o.init_walkers(W)
+    c0 = float(np.mean(o.chi2))
+    Ts = [hot * c0, cold * c0]
+    o.anneal_selfcool(2, k, n_boil=0, n_ramp=1, t_imprint=t, branch_fraction=frac, adapt=True, T_override=Ts)
+    # replay with the public pieces; block 0 at full strength
+    r = _oracle_for(tiny); r.init_walkers(W)
+    r.anneal(np.full(k, Ts[0]))
+    acc0 = int(r.acc.sum())
+    plain = _oracle_for(tiny); plain.init_walkers(W)
+    plain.anneal_selfcool(1, k, n_boil=0, n_ramp=1, t_imprint=t, branch_fraction=frac, adapt=False, T_override=Ts[:1])
+    r.branch_fraction(frac, t)
+    np.testing.assert_array_equal(r.a, plain.a)                       # scale = 1 in the first block
+    r.anneal(np.full(k, Ts[1]))
+    acc1 = int(r.acc.sum()) - acc0
+    assert 0 < acc1 < 0.8 * acc0                                      # the cold block accepts less
+    scale = acc1 / acc0
+    full = _oracle_for(tiny); full.init_walkers(W, r.a.copy()); full.chi2[:] = r.chi2; full.sweep = r.sweep
+    _, n_full, _, _ = full.branch_fraction(frac, t)
+    before = r.a.copy()
+    _, n_cut, mult, donor = r.branch_fraction(frac * scale, t * scale)
+    np.testing.assert_array_equal(r.a, o.a)                           # the protocol did exactly this
+    assert n_cut < n_full and abs(n_cut - frac * scale * W) <= 0.02 * W + 1
+    rec = np.flatnonzero(mult == 0)
+    if rec.size:                                                      # imprint strength t * scale (Eq. 26)
+        i = rec[0]
+        np.testing.assert_allclose(r.a[i], t * scale * before[donor[i]] + (1.0 - t * scale) * before[i], rtol=1e-13)
+
+
 # ---- f1 self-cooling (PAPER.md:160-162, :216) ------------------------------------------------------------
 def test_selfcool_rule_follows_the_papers_statements():
     """What the paper fixes: T starts at 10 starting residues (:216); it sits at chi2_ave while boiling, is ramped
