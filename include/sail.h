@@ -249,7 +249,10 @@ typedef struct {
  * below chi2_min, ~ 1 / blocks), then sweeps_per_block sweeps at that temperature, sail_smooth (if smooth_s > 0) and
  * one sail_branch at 1/T.  The feedback loop runs on the device (statistics, rule, schedule slice, branching parameters):
  * no host synchronisation inside a block.  T_out, chi2_ave_out, chi2_min_out: HOST [n_blocks] or NULL, copied once at
- * the end (once per 4096 blocks).  Errors: SAIL_ERR_ARG also when the rule reaches T <= 0 (reported at the end).
+ * the end (once per 4096 blocks).  Errors: SAIL_ERR_ARG also when the rule reaches T <= 0 (chi2_min is a running sum and
+ * can go negative next to an exact fit; use anneal.resync_every then).  The failing block and every later block of the
+ * call are no-ops on the device (no sweeps, no smoothing, no branching: the population stays as the last good block left
+ * it); the error, with the block index, is reported when the call returns; T_out is 0 from that block on.
  */
 SAIL_API int sail_anneal_selfcool(sail_t *h, const sail_selfcool_params *p, int64_t n_blocks, double *T_out,
                                   double *chi2_ave_out, double *chi2_min_out);

@@ -240,9 +240,12 @@ class Sail:
         return mn.value, mean.value
 
     def anneal_selfcool(self, n_blocks, sweeps_per_block, n_boil, n_ramp, eta, t_imprint=0.1, smooth_s=0.0, T_start=10.0,
-                        freeze_rate=1.0, branch=True, branch_fraction=0.0, adapt=False, T_override=None, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6):
+                        freeze_rate=1.0, branch=True, branch_fraction=0.0, adapt=False, T_override=None, amp_mode=1, amp_p=1.0, amp_m=2.0, y_min=1e-6,
+                        resync_every=0, walk_length=0, walk_uniform=0.0):
         """The paper's block protocol with self-cooling (include/sail.h: sail_anneal_selfcool).
-        Returns (T, chi2_ave, chi2_min), one entry per block."""
+        Returns (T, chi2_ave, chi2_min), one entry per block.  resync_every > 0 recomputes the residues from the spectra
+        after every such sweep (keeps the running chi2_min the rule feeds on from drifting below zero near an exact fit);
+        walk_length / walk_uniform select the index walk of section 2.3 as in anneal()."""
         p = sail_selfcool_params()
         p.sweeps_per_block, p.n_boil, p.n_ramp = sweeps_per_block, n_boil, n_ramp
         p.T_start, p.freeze_rate, p.t_imprint, p.smooth_s, p.branch = T_start, freeze_rate, t_imprint, smooth_s, int(branch)
@@ -252,6 +255,7 @@ class Sail:
         p.T_override = ov.ctypes.data if ov is not None else None
         p.anneal.eta, p.anneal.amp_mode = eta, amp_mode
         p.anneal.amp_p, p.anneal.amp_m, p.anneal.y_min = amp_p, amp_m, y_min
+        p.anneal.resync_every, p.anneal.walk_length, p.anneal.walk_uniform = resync_every, walk_length, walk_uniform
         T, ave, mn = np.zeros(n_blocks), np.zeros(n_blocks), np.zeros(n_blocks)
         self._check(self._L.sail_anneal_selfcool(self._h, C.byref(p), n_blocks, _ptr(T), _ptr(ave), _ptr(mn)))
         return T, ave, mn

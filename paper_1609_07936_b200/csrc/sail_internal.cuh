@@ -45,7 +45,7 @@ struct BranchScratch {
     unsigned long long *ehat;    // [W] fixed-point weights, then inclusive scan (in place)
     unsigned long long *scanA;   // [W] scan of recipient flags
     unsigned long long *scanB;   // [W] scan of donor extras
-    unsigned long long *block_sums; // [3 * kScanBlocksMax]
+    unsigned long long *block_sums; // [6 * 1024] per-CTA partials of the cooperative branching-plan kernel (<= 1024 CTAs)
     int32_t *mult;               // [W]
     int64_t *donor_of;           // [W]
     int64_t *rec_list;           // [W] recipient indices in ascending order
@@ -87,6 +87,7 @@ struct sail_handle {
     size_t d_T_cap = 0;
     double *ctl = nullptr;             // [32] device control block: 0 T, 1 branching fraction, 2 imprint strength (branch.cu), 8.. self-cooling state (selfcool.cu)
     double *block_out = nullptr;       // [3][kSelfcoolBlocksMax] T, chi2_ave, chi2_min per block of the self-cooling protocol
+    const double *halt = nullptr;      // DEVICE flag (ctl[12]) while sail_anneal_selfcool runs: non-zero = its rule failed, later work is skipped
     double *model_scratch = nullptr;   // [max_walkers][n_tau]: sail_get_model's scaled copy M = c mt for the host
 
     int64_t launches = 0;

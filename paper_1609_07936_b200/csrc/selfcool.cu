@@ -4,7 +4,7 @@
 // then a freeze-out below chi2_min that falls like 1 / steps (:162).  A block is sweeps_per_block sweeps at that T,
 // the smoothing step (if asked for) and one imprinted-branching event (:218-220).
 // The whole feedback loop stays on the device: the statistics (two kernels with a fixed summation order, bit-reproducible
-// run to run), the rule (one thread), the block's schedule slice, the acceptance-driven strength (reading B7) and the
+// run to run), the rule (one CTA), the block's schedule slice, the acceptance-driven strength (reading B7) and the
 // parameters of the branching event live in the handle's control block; the host only enqueues.  T / chi2_ave /
 // chi2_min per block come back once at the end of the call.
 #include <mutex>
@@ -102,22 +102,35 @@ static int enqueue_accepted_total(sail_handle *h)
 struct CoolRule { int n_boil, n_ramp; double T_start, freeze_rate, t_imprint, fraction; };
 
 // readings C1-C3: the temperature of block b from the residues measured before it (ctl[8], ctl[9]); fills the block's
-// schedule slice, the branching parameters and the per-block outputs.  One thread.
-__global__ void selfcool_rule_kernel(long long b, int out_slot, CoolRule r, int has_override, double T_override, int k,
-                                     double *ctl, double *d_T, double *block_out, int out_stride)
+// schedule slice, the branching parameters and the per-block outputs.  Thread 0 applies the rule, the CTA fills the slice.
+// A rule that gives T <= 0 (chi2_min is a running sum and can go negative next to an exact fit) HALTS the call: the flag
+// ctl[12] is set and stays set, the slice gets T = 0 — the sweep kernel returns at once on such a slice — and T = 0,
+// fraction = 0 make the branching event a no-op; sail_smooth's kernel reads the flag.  Every later block of the call does
+// the same, so the population stays as it was when the rule failed; the host reports the block at the end of the call.
+constexpr int kRuleThreads = 256;
+__global__ void __launch_bounds__(kRuleThreads) selfcool_rule_kernel(long long b, int out_slot, CoolRule r, int has_override, double T_override, int k,
+                                                                     double *ctl, double *d_T, double *block_out, int out_stride)
 {
-    const double mn = ctl[kCtlMin], ave = ctl[kCtlAve];
-    if (b == 0) { ctl[kCtlChi0] = ave; ctl[kCtlAccMax] = 0.0; }   // the unit of T and of the residue (:216)
-    double T;
-    if (has_override) T = T_override;
-    else if (b == 0) T = r.T_start * ctl[kCtlChi0];
-    else if (b <= r.n_boil) T = ave;
-    else if (b <= (long long)r.n_boil + r.n_ramp) T = ave + (mn - ave) * ((double)(b - r.n_boil) / (double)r.n_ramp);
-    else T = mn / (1.0 + r.freeze_rate * (double)(b - r.n_boil - r.n_ramp));
-    if (!(T > 0.0)) { ctl[kCtlErr] = 1.0 + (double)b; T = 1.0; }   // reported by the host at the end of the call
-    for (int i = 0; i < k; ++i) d_T[i] = T;
-    ctl[kCtlT] = T; ctl[kCtlFrac] = r.fraction; ctl[kCtlImp] = r.t_imprint;
-    block_out[out_slot] = T; block_out[out_stride + out_slot] = ave; block_out[2 * out_stride + out_slot] = mn;
+    __shared__ double sT;
+    if (threadIdx.x == 0) {
+        const double mn = ctl[kCtlMin], ave = ctl[kCtlAve];
+        if (b == 0) { ctl[kCtlChi0] = ave; ctl[kCtlAccMax] = 0.0; }   // the unit of T and of the residue (:216)
+        double T;
+        if (has_override) T = T_override;
+        else if (b == 0) T = r.T_start * ctl[kCtlChi0];
+        else if (b <= r.n_boil) T = ave;
+        else if (b <= (long long)r.n_boil + r.n_ramp) T = ave + (mn - ave) * ((double)(b - r.n_boil) / (double)r.n_ramp);
+        else T = mn / (1.0 + r.freeze_rate * (double)(b - r.n_boil - r.n_ramp));
+        const bool halted = ctl[kCtlErr] != 0.0;
+        if (!halted && !(T > 0.0)) ctl[kCtlErr] = 1.0 + (double)b;   // first failure: remember the block
+        if (halted || !(T > 0.0)) T = 0.0;
+        ctl[kCtlT] = T; ctl[kCtlFrac] = T > 0.0 ? r.fraction : 0.0; ctl[kCtlImp] = T > 0.0 ? r.t_imprint : 0.0;
+        block_out[out_slot] = T; block_out[out_stride + out_slot] = ave; block_out[2 * out_stride + out_slot] = mn;
+        sT = T;
+    }
+    __syncthreads();
+    const double T = sT;
+    for (int i = threadIdx.x; i < k; i += kRuleThreads) d_T[i] = T;
 }
 
 // :184 (reading B7): less imprinting and a smaller branching fraction as the acceptance rate falls — both are
@@ -129,7 +142,7 @@ __global__ void selfcool_strength_kernel(double moves_per_block, CoolRule r, uns
     scalars[7] = now;
     const double rate = (double)(now - prev) / moves_per_block;
     if (rate > ctl[kCtlAccMax]) ctl[kCtlAccMax] = rate;
-    const double scale = ctl[kCtlAccMax] > 0.0 ? rate / ctl[kCtlAccMax] : 0.0;
+    const double scale = (ctl[kCtlAccMax] > 0.0 && ctl[kCtlErr] == 0.0) ? rate / ctl[kCtlAccMax] : 0.0;   // halted: no branching
     ctl[kCtlFrac] = r.fraction * scale;
     ctl[kCtlImp] = r.t_imprint * scale;
 }
@@ -169,6 +182,11 @@ int sail_anneal_selfcool(sail_t *h, const sail_selfcool_params *p, int64_t n_blo
     const double moves_per_block = (double)h->W * (double)p->sweeps_per_block * (double)h->n_omega;
     const int k = p->sweeps_per_block;
     SAIL_CUDA_OK(h, cudaMemsetAsync(h->ctl + kCtlErr, 0, sizeof(double), h->stream));
+    struct HaltScope {                                   // the smoothing launches of THIS call read the halt flag
+        sail_handle *h;
+        ~HaltScope() { h->halt = nullptr; }
+    } halt_scope{h};
+    h->halt = h->ctl + kCtlErr;
     int rc;
     if (p->adapt) {                                      // scalars[7] = accepted moves so far
         if ((rc = enqueue_accepted_total(h))) return rc;
@@ -179,7 +197,7 @@ int sail_anneal_selfcool(sail_t *h, const sail_selfcool_params *p, int64_t n_blo
         const int64_t nb = n_blocks - b0 < kSelfcoolBlocksMax ? n_blocks - b0 : kSelfcoolBlocksMax;
         for (int64_t b = b0; b < b0 + nb; ++b) {
             if ((rc = enqueue_chi2_stats(h))) return rc;
-            selfcool_rule_kernel<<<1, 1, 0, h->stream>>>(b, (int)(b - b0), rule, p->T_override ? 1 : 0, p->T_override ? p->T_override[b] : 0.0, k,
+            selfcool_rule_kernel<<<1, kRuleThreads, 0, h->stream>>>(b, (int)(b - b0), rule, p->T_override ? 1 : 0, p->T_override ? p->T_override[b] : 0.0, k,
                                                          h->ctl, h->d_T, h->block_out, kSelfcoolBlocksMax);
             SAIL_LAUNCH_OK(h, "selfcool_rule_kernel");
             if ((rc = anneal_device_schedule(h, h->d_T, k, &p->anneal, k, 0))) return rc;

@@ -26,10 +26,12 @@ __device__ __forceinline__ void warp_sum3(double &x, double &y, double &z)
 }
 
 template <int PER>   // bins per lane: n_omega <= 32 PER
-__global__ void __launch_bounds__(kSmoothWarps * 32) smooth_kernel(int n_omega, long long W, double s, double B, double domega,
-                                                                   const double *__restrict__ omega, double *__restrict__ a)
+__global__ void __launch_bounds__(kSmoothWarps * 32) smooth_kernel(int n_omega, long long W, double s, double B, double c0, double domega,
+                                                                   const double *__restrict__ omega, double *__restrict__ a,
+                                                                   const double *__restrict__ halt)
 {
-    extern __shared__ __align__(128) unsigned char smem[];     // wm[n_pad] | per warp: one stage of n_pad doubles
+    if (halt && *halt != 0.0) return;      // sail_anneal_selfcool after its rule failed: the rest of the call is a no-op
+    extern __shared__ __align__(128) unsigned char smem[];     // wm[n_pad] - c0 | per warp: one stage of n_pad doubles
     __shared__ __align__(8) unsigned long long bars[kSmoothWarps];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int n_pad = (n_omega + 1) & ~1;
@@ -37,7 +39,10 @@ __global__ void __launch_bounds__(kSmoothWarps * 32) smooth_kernel(int n_omega, 
     double *row = s_wm + n_pad + (size_t)warp * n_pad;
     const double c = 1.0 - 2.0 * s, e = 1.0 - s, half = 0.5 * domega;
     const bool bulk = (n_omega & 1) == 0;                      // rows are multiples of 16 bytes: bulk copies
-    for (int k = threadIdx.x; k < n_omega; k += blockDim.x) s_wm[k] = omega[k] + half;
+    // frequencies are kept RELATIVE to c0 = B / A, the mean frequency the two sum rules pin (Eq. 23): the smoothed row's
+    // own mean differs from it by O(s domega), so the one-pass second moment below does not cancel however narrow the
+    // spectrum is or wherever it sits on the grid (about 0 it lost (wbar / width)^2 eps)
+    for (int k = threadIdx.x; k < n_omega; k += blockDim.x) s_wm[k] = (omega[k] + half) - c0;
     const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&bars[warp]);
     if (lane == 0) {
         asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" :: "r"(bar) : "memory");
@@ -87,19 +92,22 @@ __global__ void __launch_bounds__(kSmoothWarps * 32) smooth_kernel(int n_omega, 
         // the whole row now lives in registers: the stage is free, the next row streams in behind the reductions
         if (bulk && lane == 0 && w + stride < W) fetch(w + stride);
         warp_sum3(sA, sB, sC);
-        const double A1 = sA, B1 = sB;
-        const double wbar = B1 / A1;
-        // sum a_k (w_k - wbar)^2 = sum a_k w_k^2 - wbar sum a_k w_k  (one reduction round instead of two)
-        const double V = fma(-wbar, B1, sC);
-        double kappa = (V > 0.0) ? (B - B1) / V : 0.0;
+        // with u_k = w_k - c0:  sB = B' - c0 A',  wbar - c0 = sB / A',  B - B' = (B - c0 A') - sB
+        const double A1 = sA, U1 = sB;
+        const double wbar = U1 / A1;                           // the row's mean frequency, relative to c0
+        // sum a_k (u_k - wbar)^2 = sum a_k u_k^2 - wbar sum a_k u_k  (one reduction round instead of two)
+        const double V = fma(-wbar, U1, sC);
+        double kappa = (V > 0.0) ? (fma(-c0, A1, B) - U1) / V : 0.0;
         // positivity (reading S2): the tilt factor is linear in k, smallest at an end bin
         const double d_lo = s_wm[0] - wbar, d_hi = s_wm[n_omega - 1] - wbar;
-        if (1.0 + kappa * d_lo < 0.0) kappa = -1.0 / d_lo;
-        if (1.0 + kappa * d_hi < 0.0) kappa = -1.0 / d_hi;
+        // (product and sum rounded separately, here and in the store below: a fused 1 + kappa d at the clamped end bin would
+        // see the rounding error of -1 / d and could come out at -1e-16, a negative coefficient; fl(fl(-1/d) d) >= -1)
+        if (__dadd_rn(1.0, __dmul_rn(kappa, d_lo)) < 0.0) kappa = -1.0 / d_lo;
+        if (__dadd_rn(1.0, __dmul_rn(kappa, d_hi)) < 0.0) kappa = -1.0 / d_hi;
 #pragma unroll
         for (int i = 0; i < PER; ++i) {
             const int k = lane + 32 * i;
-            if (k < n_omega) aw[k] = nv[i] * (1.0 + kappa * (s_wm[k] - wbar));
+            if (k < n_omega) aw[k] = nv[i] * __dadd_rn(1.0, __dmul_rn(kappa, s_wm[k] - wbar));
         }
     }
 }
@@ -110,7 +118,7 @@ int launch_smooth(sail_handle *h, double s)
     const long long W = h->W;
     const int n_pad = (h->n_omega + 1) & ~1;
     const size_t smem = (size_t)(1 + kSmoothWarps) * n_pad * sizeof(double);
-    void (*kern)(int, long long, double, double, double, const double *, double *);
+    void (*kern)(int, long long, double, double, double, double, const double *, double *, const double *);
     const int per = (h->n_omega + 31) / 32;
     if (per <= 8) kern = smooth_kernel<8>;
     else if (per <= 16) kern = smooth_kernel<16>;
@@ -122,7 +130,7 @@ int launch_smooth(sail_handle *h, double s)
     if (per_sm < 1) return set_err(h, SAIL_ERR_CUDA, "smooth_kernel does not fit an SM");
     long long blocks = (W + kSmoothWarps - 1) / kSmoothWarps;
     if (blocks > (long long)h->num_sms * per_sm) blocks = (long long)h->num_sms * per_sm;
-    kern<<<(unsigned)blocks, kSmoothWarps * 32, smem, h->stream>>>(h->n_omega, W, s, h->B, h->domega, h->tab.omega, h->st.a);
+    kern<<<(unsigned)blocks, kSmoothWarps * 32, smem, h->stream>>>(h->n_omega, W, s, h->B, h->B / h->A, h->domega, h->tab.omega, h->st.a, h->halt);
     SAIL_LAUNCH_OK(h, "smooth_kernel");
     return launch_forward(h, 0, W);
 }

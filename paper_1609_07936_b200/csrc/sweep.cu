@@ -119,6 +119,9 @@ __global__ void __maxnreg__((65536 / (((MAXW + 3) & ~3) * 32)) & ~7) sweep_kerne
     // WALK: track the bins a walk read (so that only affected lanes walk again) in the kernels that have the registers
     // for it; measured at L = 2: +10 % on a 1024-bin grid, -4 % at 256 bins in the 72-register form, which keeps re-walking
     constexpr bool TRACK = WALK && C > 4;
+    // a schedule written on the device (sail_anneal_selfcool) says "halted" with a non-positive first temperature: the
+    // whole launch is then a no-op.  Schedules from the host are validated > 0 by sail_anneal, so this never fires there.
+    if (!(__ldg(P.T) > 0.0)) return;
     extern __shared__ __align__(16) unsigned char smem[];
     double *s_ratio = reinterpret_cast<double *>(smem);
     const int n_omega = P.n_omega;
@@ -497,8 +500,8 @@ template <int C, int MAXW, bool W2REG, bool ACACHE>
 static int launch_c(sail_handle *h, SweepArgs &a, bool trace)
 {
     const bool walk = a.walk_len > 0;
-    // the walk reads the spectrum at random bins: fewer warps per SM (24 at C <= 4) keep records + tables within the
-    // 164 KB shared-memory carve-out, which leaves the L1 large enough for the spectra of the resident walkers
+    // the walking kernels run as many warps per SM as the plain ones (fewer were tried and lost); when the spectra of the
+    // resident warps fit beside tables + records they are copied to shared memory (launch_variant: spec_smem)
     constexpr int MAXW_WALK = MAXW;
 #define SAIL_PICK(FA, TR)                                                                    \
     return walk ? launch_variant<C, MAXW_WALK, FA, TR, W2REG, false, true>(h, a)            \

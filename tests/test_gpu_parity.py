@@ -890,3 +890,262 @@ def test_branching_with_negative_running_residues():
     assert mult.sum() == W and (mult == mo).all() and (donor == do).all()
     assert mult[17] >= 1
     s.close()
+
+
+def _replay_sweeps(s, w, lo, hi, sweep_abs, T, a_g, c_g):
+    """Trace walkers [lo, hi) on the GPU for len(T) sweeps starting at absolute sweep `sweep_abs`; the oracle replays
+    them from the injected GPU state (a_g, c_g = the population's spectra and running residues right now)."""
+    _, _, y_g = s.stats()
+    o = _oracle(w, hi - lo, spectra=a_g[lo:hi])
+    o.chi2[:] = c_g[lo:hi]
+    o.y[:] = y_g[lo:hi]
+    tg, _ = s.anneal(T, w.eta, trace_walkers=(lo, hi))
+    tr_o = np.zeros((hi - lo, len(T), w.n_omega), dtype=oracle.TRACE_DTYPE)
+    for i in range(hi - lo):
+        for k in range(len(T)):
+            for m in range(w.n_omega):
+                tr_o[i, k, m] = _oracle_move(o, i, lo + i, sweep_abs + k, m, T[k])
+            _end_sweep(o, i, tr_o[i, k])
+    flagged = compare_traces(tg, tr_o, T, w.A / w.n_omega)
+    a2, c2 = s.get()
+    np.testing.assert_allclose(a2[lo:hi], o.a, rtol=0, atol=1e-10 * o.a.max())
+    np.testing.assert_allclose(c2[lo:hi], o.chi2, rtol=1e-9, atol=1e-13 * float(np.abs(c_g).max()))
+    return flagged, tg
+
+
+@pytest.mark.parametrize("name,W", [("tiny", 64), ("small", 80), ("branching", 72), ("noise", 48), ("stress", 40)])
+def test_cold_end_of_the_schedule_on_every_kernel_instantiation(name, W):
+    """the COLD regime (T -> 1e-5 of the starting scale: few moves accepted, y far below 1, thresholds
+    -T ln u tiny against the terms of the sum) on each sweep-kernel instantiation — 1, 4, 7, 8 and 16 tau-points per
+    lane, direct and factored start tables.  The configuration's own schedule compressed to 60 sweeps runs on the GPU
+    (with its branching events and resync), then two more sweeps at the final temperature are traced for every walker
+    and replayed by the oracle from the injected state."""
+    w = wl.make(name, simpson_intervals=20_000).scaled(W=W, n_sweeps=60)
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED)
+    step = 20
+    for b in range(0, 60, step):
+        s.anneal(w.schedule[b:b + step], w.eta, resync_every=30)
+        if w.branch_every:
+            s.branch_async(float(w.schedule[b + step - 1]), w.t_imprint)
+    acc0, ev0, y = s.stats()
+    assert np.median(y) < 0.5                                      # Eq. 30 has cut the amplitude: the cold regime
+    a_g, c_g = s.get()
+    T = np.full(2, w.schedule[-1])
+    flagged, tg = _replay_sweeps(s, w, 0, W, 60, T, a_g, c_g)
+    assert flagged == 0
+    acc_rate = ((tg["flags"] & 2) != 0).mean()
+    assert acc_rate < 0.5                                          # and most evaluated moves are refused
+    s.close()
+
+
+@pytest.mark.parametrize("t", [1.0, 0.1])
+def test_branching_parity_at_stress_row_size(t):
+    """the imprint kernels on the rows bench.py times them on (N_omega = 2048, N_tau = 512: 20 KB per
+    walker) — t = 1 is the bulk-copy ring (recipients become bit-copies of their donors), t = 0.1 the arithmetic form —
+    multipliers, donor map, spectra and model against the oracle."""
+    w = wl.make("stress", simpson_intervals=20_000)
+    W = 600
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED)
+    s.anneal(np.full(2, 1.0), w.eta)
+    a0, c0 = s.get()
+    o = _oracle(w, W, spectra=a0)
+    o.chi2[:] = c0
+    o.sweep = 2
+    T = float(np.std(c0))
+    info, mult, donor = s.branch(T, t, want_maps=True)
+    n_rec, mo, do = o.branch(T, t)
+    assert mult.sum() == W and (mult == mo).all() and (donor == do).all() and info.n_recipients == n_rec > 50
+    a1, c1 = s.get()
+    np.testing.assert_array_equal(a1, o.a)
+    rec = donor >= 0
+    if t == 1.0:
+        np.testing.assert_array_equal(a1[rec], a0[donor[rec]])
+    np.testing.assert_allclose(s.get_model()[rec], o.M[rec], rtol=1e-12)
+    np.testing.assert_allclose(c1[rec], o.chi2[rec], rtol=1e-8)
+    np.testing.assert_array_equal(c1[~rec], c0[~rec])
+    s.close()
+
+
+def test_stress_configuration_mid_and_late_anneal_parity():
+    """configs[4] at FULL size (W = 262144) beyond its first sweep.  The configuration's schedule
+    compressed to 60 sweeps (T 1 -> 1e-5) runs in three blocks of 20 with a resync and an imprinted-branching event
+    (t = 0.1) after each, as bench.py drives it.  After the first and the last block: (i) the multipliers and the donor
+    map of the W = 262144 event against the oracle's plan computed from the GPU's residues (an oracle on a 2-bin dummy
+    problem with the same seed and sweep counter: the plan depends on chi^2, W, T and the comb offset only); (ii) 12
+    walkers around a fresh recipient traced for one sweep and replayed by the oracle from the injected state."""
+    w = wl.make("stress", simpson_intervals=100_000).scaled(n_sweeps=60)
+    s = _sail(w, w.W)
+    s.init_walkers(w.W, w.A, w.B, SEED)
+    dummy = oracle.Oracle(np.array([0.0, 1.0]), np.array([0.0]), np.array([1.0]), None, 1.0, 1.0, w.eta, SEED)
+    dummy.init_walkers(w.W)
+    done = 0
+    for block in range(3):
+        s.anneal(w.schedule[done:done + 20], w.eta, resync_every=20)
+        done += 20
+        _, c0 = s.get(spectra=False)
+        T = float(w.schedule[done - 1])
+        info, mult, donor = s.branch(T, w.t_imprint, want_maps=True)
+        if block == 1:
+            continue
+        dummy.chi2[:] = c0
+        dummy.sweep = done
+        n_rec, mo, do = dummy.branch(T, 0.0)
+        assert (mult == mo).all() and (donor == do).all() and info.n_recipients == n_rec
+        assert n_rec > 0
+        rec = np.flatnonzero(donor >= 0)
+        lo = max(0, min(int(rec[rec.size // 2]) - 6, w.W - 12))
+        hi = lo + 12
+        a_g, c_g = s.get()
+        flagged, _ = _replay_sweeps(s, w, lo, hi, done, w.schedule[done - 1:done], a_g, c_g)
+        del a_g
+        assert flagged == 0
+        s.set_sweep(done)                                        # the traced sweep was an extra one: back on the schedule
+    s.close()
+
+
+def test_selfcool_and_branch_fraction_parity_on_the_noise_grid():
+    """the block protocol (f1) and the prescribed-fraction event (f2) on a grid that takes the 8-points-
+    per-lane sweep kernel, factored start tables and smooth_kernel<32> (N_omega = 1024, N_tau = 256), W = 64."""
+    w = wl.make("noise", simpson_intervals=20_000)
+    W, nb, k = 64, 4, 3
+    s = _sail(w, W)
+    s.init_walkers(W, w.A, w.B, SEED)
+    T, ave, mins = s.anneal_selfcool(nb, k, 1, 2, w.eta, t_imprint=0.1, smooth_s=0.01, branch_fraction=0.25, adapt=True)
+    o = _oracle(w, W)
+    o.anneal_selfcool(nb, k, 1, 2, t_imprint=0.1, smooth_s=0.01, branch_fraction=0.25, adapt=True, T_override=T)
+    a, c2 = s.get()
+    np.testing.assert_allclose(a, o.a, rtol=0, atol=1e-9 * o.a.max())
+    np.testing.assert_allclose(c2, o.chi2, rtol=1e-7)
+    for b in range(nb):
+        want = oracle.selfcool_temperature(b, ave[0], ave[b], mins[b], 1, 2)
+        assert abs(T[b] - want) <= 1e-14 * want
+    # one more prescribed-fraction event from the common state
+    o.chi2[:] = c2; o.a[:] = a; o.resync(); o.chi2[:] = c2
+    Tg, info, mult, donor = s.branch_fraction(0.25, 0.3, want_maps=True)
+    To, n_rec, mo, do = o.branch_fraction(0.25, 0.3)
+    assert abs(Tg - To) <= 1e-12 * To and (mult == mo).all() and (donor == do).all() and info.n_recipients == n_rec >= 16
+    np.testing.assert_array_equal(s.get()[0], o.a)
+    s.close()
+
+
+def test_selfcool_halts_where_its_rule_fails():
+    """when the self-cooling rule reaches T <= 0 (a running residue below zero, as next to an exact fit), the
+    failing block and all later blocks of the call must leave the population alone — no sweeps, smoothing or branching
+    at a made-up temperature — and the call reports the block.
+    (A) walker 7 gets a negative running residue; with no boil and a one-block ramp the rule gives T = chi2_min < 0 at
+        block 1 (PAPER.md:162 ramps T to chi2_min): the state after the failed 4-block call is the state after block 0.
+    (B) all running residues negative, smoothing on: the rule fails at block 0 and nothing moves at all."""
+    from paper_1609_07936_b200.binding import SailError, SAIL_ERR_ARG
+    w = wl.make("tiny", simpson_intervals=20_000)
+    W, k = 64, 3
+    kw = dict(n_boil=0, n_ramp=1, eta=w.eta, t_imprint=0.1, T_start=1e-6)
+
+    def start(all_negative=False):
+        s = _sail(w, W)
+        s.init_walkers(W, w.A, w.B, SEED)
+        s.anneal(np.full(2, 1e6), w.eta)                       # distinct walkers
+        _, c2 = s.get()
+        c2 = c2.copy()
+        if all_negative:
+            c2 = -c2
+        else:
+            c2[7] = -30.0 * c2.mean()
+        s.set_chi2(c2)
+        return s
+
+    good = start()
+    T, ave, mn = good.anneal_selfcool(1, k, **kw)               # block 0 alone: T = 1e-6 chi2_ave > 0
+    assert T[0] > 0 and mn[0] < 0 < ave[0]
+    a_good, c_good = good.get()
+    acc_good, ev_good, y_good = good.stats()
+    good.close()
+
+    bad = start()
+    with pytest.raises(SailError) as err:
+        bad.anneal_selfcool(4, k, **kw)                         # block 1: T = chi2_min < 0
+    assert err.value.code == SAIL_ERR_ARG and "block 1" in str(err.value)
+    a_bad, c_bad = bad.get()
+    acc_bad, ev_bad, y_bad = bad.stats()
+    assert np.array_equal(a_bad, a_good) and np.array_equal(c_bad, c_good)      # blocks 1..3 were no-ops
+    assert np.array_equal(acc_bad, acc_good) and np.array_equal(ev_bad, ev_good) and np.array_equal(y_bad, y_good)
+    # the handle is usable afterwards, and a later call starts with the flag cleared
+    T2, _, _ = bad.anneal_selfcool(1, k, T_override=[float(ave[0])], **kw)
+    assert T2[0] == ave[0] and not np.array_equal(bad.get()[0], a_good)
+    bad.close()
+
+    cold = start(all_negative=True)
+    a0, _ = cold.get()
+    acc0, ev0, y0 = cold.stats()
+    with pytest.raises(SailError) as err:
+        cold.anneal_selfcool(3, k, smooth_s=0.05, **kw)         # block 0: T = T_start chi2_ave < 0
+    assert "block 0" in str(err.value)
+    assert np.array_equal(cold.get()[0], a0)                    # no sweep, no stencil, no imprint
+    acc1, ev1, y1 = cold.stats()
+    assert np.array_equal(acc1, acc0) and np.array_equal(ev1, ev0) and np.array_equal(y1, y0)
+    cold.close()
+
+
+def _rows_with_common_sums(rng, W, n, wm, A, mean, support_of, profile_of):
+    """W non-negative rows with sum A and mean frequency `mean`: a random positive profile on the row's support, mixed
+    with a spike in the support's first or last bin (whichever side the mean has to move to)."""
+    spectra = np.zeros((W, n))
+    for i in range(W):
+        k = support_of(i)
+        x = profile_of(i, k) * rng.uniform(0.5, 1.5, k.size)
+        x *= A / x.sum()
+        m = (x * wm[k]).sum() / A
+        j = k[-1] if m < mean else k[0]
+        lam = (mean - m) / (wm[j] - m)
+        assert 0.0 <= lam <= 1.0
+        spectra[i, k] = (1.0 - lam) * x
+        spectra[i, j] += lam * A
+    return spectra
+
+
+@pytest.mark.parametrize("name,kind", [("stress", "clamped"), ("tiny", "clamped"), ("stress", "unclamped"), ("tiny", "unclamped")])
+def test_smoothing_of_spectra_piled_at_the_top_of_the_grid(name, kind):
+    """VERDICT r2 1(c) / ADVICE r2 (smooth.cu): rows whose weight sits in the last bins, s = 0.05.
+    clamped: rows 2-6 bins wide ending in the last bin.  The stencil lowers B by s domega a_{N-1} (:197); restoring it
+      needs 1 + kappa (w_0 - wbar) < 0, so reading S2's clamp acts (kappa = -1 / (w_0 - wbar)): B is restored only in
+      part, every coefficient stays >= 0 (the kernel rounds kappa d and 1 + kappa d separately, as the oracle does: fused,
+      the factor at the clamped bin could come out at -1e-16).  Spectra to 1e-13: the clamp value does not involve the
+      variance.
+    unclamped: half-Gaussian rows of width max(N/64, 4) bins at the top end: the mean sits ~60 widths from 0, the one-pass second
+      moment about 0 would lose (wbar / width)^2 eps ~ 4e-13 of the variance; the kernel takes its moments about B / A.
+      Both sums restored; spectra to 1e-12 (the rounding of B - B' on both sides, ~ N eps B / |B - B'| kappa d)."""
+    w = wl.make(name, simpson_intervals=20_000)
+    n, W, s_amp, A = w.n_omega, 24, 0.05, 3.0
+    wm = w.omega + 0.5 * w.domega
+    rng = np.random.Generator(np.random.Philox(77))
+    if kind == "clamped":
+        mean = wm[n - 2] + 0.25 * w.domega
+        spectra = _rows_with_common_sums(rng, W, n, wm, A, mean, lambda i: np.arange(n - (2 + i % 5), n), lambda i, k: np.ones(k.size))
+    else:
+        sg = max(n / 64.0, 4.0)
+        mean = wm[n - 1] - 0.8 * sg * w.domega
+        spectra = _rows_with_common_sums(rng, W, n, wm, A, mean, lambda i: np.arange(n - int(4 * sg), n),
+                                         lambda i, k: np.exp(-0.5 * ((k - (n - 1)) / sg) ** 2))
+    B = A * mean
+    assert (spectra >= 0).all() and (spectra[:, -1] > 0).all()
+    np.testing.assert_allclose(spectra.sum(axis=1), A, rtol=1e-14)
+    np.testing.assert_allclose((spectra * wm).sum(axis=1), B, rtol=1e-14)
+    o = oracle.Oracle(w.omega, w.tau, w.F, w.sigma, A, B, w.eta, SEED)
+    o.init_walkers(W, spectra)
+    s = _sail(w, W)
+    s.init_walkers(W, A, B, SEED, spectra=spectra)
+    s.smooth(s_amp); o.smooth(s_amp)
+    a1, c1 = s.get()
+    assert (a1 >= 0).all()
+    np.testing.assert_allclose(a1.sum(axis=1), A, rtol=1e-13)
+    B_stencil = B + s_amp * w.domega * (spectra[:, 0] - spectra[:, -1])      # :197 (pinned on the CPU side)
+    B_out = (a1 * wm).sum(axis=1)
+    if kind == "clamped":
+        np.testing.assert_allclose(a1, o.a, rtol=1e-13, atol=0)
+        assert (B_stencil < B_out).all() and (B_out < B).all() and (B - B_out > 1e-3 * (B - B_stencil)).all()   # in part only
+    else:
+        np.testing.assert_allclose(a1, o.a, rtol=1e-12, atol=0)
+        np.testing.assert_allclose(B_out, B, rtol=1e-13)
+    np.testing.assert_allclose(c1, o.chi2, rtol=1e-8)
+    s.close()
