@@ -203,7 +203,7 @@ class Oracle:
     def anneal_selfcool(self, n_blocks, sweeps_per_block, n_boil, n_ramp, t_imprint=0.1, smooth_s=0.0,
                         T_start=10.0, freeze_rate=1.0, T_override=None, branch_fraction=0.0, adapt=False):
         """The paper's block protocol (:218-220) with self-cooling: per block, T from the population's residues, then
-        sweeps_per_block sweeps at that T, smoothing (if smooth_s > 0), one branching event at 1/T (or, with
+        smoothing (if smooth_s > 0; :199), sweeps_per_block sweeps at that T, one branching event at 1/T (or, with
         branch_fraction > 0, at the 1/T that gives that fraction of walkers multiplier zero: the paper's 1/4, :220).  T_override[b]
         replaces the rule (used by the parity tests to drive both sides with the same temperatures).
         Returns (T, chi2_ave, chi2_min) per block."""
@@ -216,9 +216,12 @@ class Oracle:
             if T_override is not None:
                 T = float(T_override[b])
             Ts.append(T); aves.append(ave); mins.append(mn)
-            self.anneal(np.full(sweeps_per_block, T))
+            # reading C3 as amended in round 3 ("Once the transforms are smoothed and renormalized, they
+            # undergo Metropolis updates and branching.  The process is then repeated."): smoothing opens the block, so
+            # the k sweeps relax what the stencil damaged before the branching weighs the walkers
             if smooth_s > 0.0:
                 self.smooth(smooth_s)
+            self.anneal(np.full(sweeps_per_block, T))
             scale = 1.0
             if adapt:       # :184, reading B7: strength follows the block's acceptance rate relative to the largest seen
                 acc_now = int(self.acc.sum())

@@ -653,6 +653,30 @@ def test_selfcool_protocol_runs_blocks_of_sweeps_branching_and_smoothing(tiny):
     np.testing.assert_allclose((o.a * wm).sum(axis=1), tiny.B, rtol=1e-11)
 
 
+def test_selfcool_block_is_smoothing_then_sweeps_then_branching(tiny):
+    """"Once the transforms are smoothed and renormalized, they undergo Metropolis updates and branching.
+    The process is then repeated."  One block of the protocol is therefore smooth -> k sweeps -> branch, in that order:
+    replayed with the three public steps it gives the same state bit for bit, and the other order (sweeps -> smooth ->
+    branch, the build's reading until round 2) does not."""
+    W, k, s_amp, t = 24, 3, 0.05, 0.1
+    o = _oracle_for(tiny); o.init_walkers(W)
+    o.anneal(tiny.schedule[:4])                                      # a population that is not flat
+    start_a, start_c, start_y, start_sweep = o.a.copy(), o.chi2.copy(), o.y.copy(), o.sweep
+
+    def fresh():
+        r = _oracle_for(tiny); r.init_walkers(W, start_a.copy())
+        r.chi2[:] = start_c; r.y[:] = start_y; r.sweep = start_sweep
+        return r
+
+    p = fresh()
+    T, _, _ = p.anneal_selfcool(1, k, n_boil=0, n_ramp=1, t_imprint=t, smooth_s=s_amp)
+    a = fresh(); a.smooth(s_amp); a.anneal(np.full(k, T[0])); a.branch(T[0], t)
+    b = fresh(); b.anneal(np.full(k, T[0])); b.smooth(s_amp); b.branch(T[0], t)
+    np.testing.assert_array_equal(p.a, a.a)
+    np.testing.assert_array_equal(p.chi2, a.chi2)
+    assert not np.array_equal(p.a, b.a)
+
+
 # ---- f2 branching fraction (PAPER.md:174, :220) -----------------------------------------------------------
 def test_branch_fraction_finds_the_temperature_that_kills_the_asked_fraction(tiny):
     """:174 'Delta is found numerically such that a given fraction of walkers is assigned a zero multiplier'.
