@@ -232,7 +232,7 @@ typedef struct {
     double  T_start;            /* temperature of block 0 in units of the starting residue (paper: 10, :216)        */
     double  freeze_rate;        /* freeze-out: T = chi2_min / (1 + freeze_rate * blocks since the ramp ended)       */
     double  t_imprint;          /* imprint strength of the branching after every block (paper: 0.1, :220)          */
-    double  smooth_s;           /* smoothing amplitude applied before the branching; 0 = no smoothing (:190)        */
+    double  smooth_s;           /* smoothing amplitude applied at the start of every block; 0 = no smoothing (:190, :199) */
     int32_t branch;             /* 0: no branching                                                                  */
     int32_t adapt;              /* 1: imprint strength and branching fraction of a block are multiplied by the block's
                                  * acceptance rate relative to the largest one seen so far (:184, reading B7)          */
@@ -246,7 +246,8 @@ typedef struct {
  * sail_anneal_selfcool — n_blocks blocks of the paper's protocol (:218-220) with the self-cooling schedule of
  * section 2.4 (:160-162): before each block the residues chi2_ave, chi2_min are measured (sail_chi2_stats), the block's
  * temperature follows from them (block 0: T_start starting residues; boil: chi2_ave; ramp: linear to chi2_min; freeze-out:
- * below chi2_min, ~ 1 / blocks), then sweeps_per_block sweeps at that temperature, sail_smooth (if smooth_s > 0) and
+ * below chi2_min, ~ 1 / blocks), then sail_smooth (if smooth_s > 0; :199 "Once the transforms are smoothed and
+ * renormalized, they undergo Metropolis updates and branching"), sweeps_per_block sweeps at that temperature and
  * one sail_branch at 1/T.  The feedback loop runs on the device (statistics, rule, schedule slice, branching parameters):
  * no host synchronisation inside a block.  T_out, chi2_ave_out, chi2_min_out: HOST [n_blocks] or NULL, copied once at
  * the end (once per 4096 blocks).  Errors: SAIL_ERR_ARG also when the rule reaches T <= 0 (chi2_min is a running sum and

@@ -26,7 +26,9 @@
  *                       (zeros(T) >= n0 > zeros(T (1 + 1e-9))); the bracketing path itself (B6) is unpinned
  *   orc_stencil         cosine (DCT-II) modes are eigenvectors with eigenvalue 1 - 2s(1 - cos(pi n/N));
  *                       sum a kept, sum a w^m shifted by s domega (a_0 - a_{N-1}); s = 0 identity
- *   orc_smooth          A, B restored to 1e-13, positivity; the choice of renormalisation (S2) is unpinned
+ *   orc_smooth          A, B restored to 1e-13, positivity; the clamp branch: no negative coefficient, factor 0 at the
+ *                       clamped end bin, sum a kept, B moved towards its target; the choice of renormalisation (S2)
+ *                       itself is unpinned
  * Parity unpinned (paper silent; inputs identical on both sides): the width/shape of the
  * random move rho (eta, uniform), y_min, the acceptance window of Eq. 30, the comb choice of xi.
  */

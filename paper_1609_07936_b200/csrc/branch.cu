@@ -253,9 +253,8 @@ __global__ void __launch_bounds__(kPlanThreads) branch_plan_kernel(const PlanArg
     }
 }
 
-// Eq. 26: a(l1) <- t a(l2) + (1-t) a(l1) for spectrum and model (linearity); chi^2 of the
-// recipient from its new model.  One CTA per recipient, 128-bit accesses when rows are 16-byte aligned.
-// One CTA per recipient: a and mt of the recipient become t * donor + (1 - t) * self (two roundings per product
+// Eq. 26: a(l1) <- t a(l2) + (1-t) a(l1) for spectrum and model (linearity).  One CTA per recipient,
+// 128-bit accesses when rows are 16-byte aligned: a and mt of the recipient become t * donor + (1 - t) * self (two roundings per product
 // and one per sum, exactly the definition), chi^2 is recomputed from the new model.  COPY (t == 1): t * z + 0 * x
 // is z bit for bit, so the recipient is not read at all (two streams instead of three).  All loads of a CTA's
 // pass are issued before its first store (8 x 16 B per thread in flight).
@@ -460,15 +459,9 @@ static int branch_imprint(sail_handle *h, double t_imprint, const double *t_dev)
     if ((h->n_omega & 1) == 0 && (h->n_tau & 1) == 0 && tma_smem <= 96 * 1024 && copy) {
         const int per_sm = (int)((200 * 1024) / (tma_smem + 1024)) < 8 ? (int)((200 * 1024) / (tma_smem + 1024)) : 8;
         const int tblocks = (int)(W < (long long)h->num_sms * per_sm ? W : (long long)h->num_sms * per_sm);
-        if (copy) {
-            SAIL_CUDA_OK(h, cudaFuncSetAttribute(imprint_tma_kernel<true, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tma_smem));
-            imprint_tma_kernel<true, 3><<<tblocks, 128, tma_smem, h->stream>>>(h->n_omega, h->n_tau, t_imprint, b.rec_list, b.donor_of, b.scalars,
-                                                                              h->st.a, h->st.mt, h->st.chi2, h->tab.Wj, h->tab.fj);
-        } else {
-            SAIL_CUDA_OK(h, cudaFuncSetAttribute(imprint_tma_kernel<false, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tma_smem));
-            imprint_tma_kernel<false, 2><<<tblocks, 128, tma_smem, h->stream>>>(h->n_omega, h->n_tau, t_imprint, b.rec_list, b.donor_of, b.scalars,
-                                                                               h->st.a, h->st.mt, h->st.chi2, h->tab.Wj, h->tab.fj);
-        }
+        SAIL_CUDA_OK(h, cudaFuncSetAttribute(imprint_tma_kernel<true, 3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)tma_smem));
+        imprint_tma_kernel<true, 3><<<tblocks, 128, tma_smem, h->stream>>>(h->n_omega, h->n_tau, t_imprint, b.rec_list, b.donor_of, b.scalars,
+                                                                          h->st.a, h->st.mt, h->st.chi2, h->tab.Wj, h->tab.fj);
         SAIL_LAUNCH_OK(h, "imprint_tma_kernel");
         return SAIL_OK;
     }

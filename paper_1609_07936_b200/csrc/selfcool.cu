@@ -1,8 +1,8 @@
 // selfcool.cu — population statistics and the self-cooling block protocol (PAPER.md:160-162,
 // :216-220; readings C1-C3 in DESIGN.md §2).  The temperature of a block follows the residues the population has
 // reached: T = 10 starting residues for block 0 (:216), T = chi2_ave while "boiling", a linear ramp to chi2_min,
-// then a freeze-out below chi2_min that falls like 1 / steps (:162).  A block is sweeps_per_block sweeps at that T,
-// the smoothing step (if asked for) and one imprinted-branching event (:218-220).
+// then a freeze-out below chi2_min that falls like 1 / steps (:162).  A block is the smoothing step (if asked for; :199),
+// sweeps_per_block sweeps at that T and one imprinted-branching event (:218-220).
 // The whole feedback loop stays on the device: the statistics (two kernels with a fixed summation order, bit-reproducible
 // run to run), the rule (one CTA), the block's schedule slice, the acceptance-driven strength (reading B7) and the
 // parameters of the branching event live in the handle's control block; the host only enqueues.  T / chi2_ave /
@@ -200,8 +200,10 @@ int sail_anneal_selfcool(sail_t *h, const sail_selfcool_params *p, int64_t n_blo
             selfcool_rule_kernel<<<1, kRuleThreads, 0, h->stream>>>(b, (int)(b - b0), rule, p->T_override ? 1 : 0, p->T_override ? p->T_override[b] : 0.0, k,
                                                          h->ctl, h->d_T, h->block_out, kSelfcoolBlocksMax);
             SAIL_LAUNCH_OK(h, "selfcool_rule_kernel");
-            if ((rc = anneal_device_schedule(h, h->d_T, k, &p->anneal, k, 0))) return rc;
+            // reading C3 as amended (smoothed and renormalised transforms "undergo Metropolis updates and
+            // branching.  The process is then repeated."): smoothing opens the block, the k sweeps relax it, then branching
             if (p->smooth_s > 0.0 && (rc = launch_smooth(h, p->smooth_s))) return rc;
+            if ((rc = anneal_device_schedule(h, h->d_T, k, &p->anneal, k, 0))) return rc;
             if (p->adapt) {
                 if ((rc = enqueue_accepted_total(h))) return rc;
                 selfcool_strength_kernel<<<1, 1, 0, h->stream>>>(moves_per_block, rule, h->br.scalars, h->ctl);

@@ -181,27 +181,3 @@ def random_problem(seed, n_omega, n_tau, omega_max=6.0, dtau=0.07, eps=1e-3):
     w = Workload(name=f"rand{seed}", n_omega=n_omega, omega_max=omega_max, n_tau=n_tau, dtau=dtau,
                  eps=eps, noise_seed=seed, W=4, n_sweeps=4, t0=1.0, t1=0.1)
     return w.build(simpson_intervals=20_000)
-
-
-def random_positive_spectra(seed, W, n_omega, omega, domega, A, B):
-    """W random strictly-positive spectra with sums A and B (for state-injection tests).
-
-    Construction (no method code): draw positive weights, then mix with two fixed positive
-    profiles to hit both linear constraints with a positive combination when possible;
-    falls back to exponential reweighting by bisection."""
-    rng = np.random.Generator(np.random.Philox(seed))
-    wm = omega + 0.5 * domega
-    out = np.empty((W, n_omega))
-    for i in range(W):
-        base = rng.random(n_omega) + 0.05
-        lo, hi = -50.0, 50.0
-        for _ in range(200):  # tilt exp(-lam*w) so that the mean frequency is B/A
-            lam = 0.5 * (lo + hi)
-            a = base * np.exp(-lam * (wm - wm[0]))
-            if (a * wm).sum() / a.sum() > B / A:
-                lo = lam
-            else:
-                hi = lam
-        a *= A / a.sum()
-        out[i] = a
-    return out
