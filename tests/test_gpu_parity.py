@@ -1,6 +1,6 @@
 """GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the CPU oracle on the same
 seeded inputs.  Three agreement levels (BASELINE.json north_star):
-  L1  per traced move: identical p, s; rho, delta within 4 ulp; |dchi2_gpu - dchi2_cpu| <= 1e-12 * l1
+  L1  per traced move: identical p, s; rho, delta within 4 ulp; |dchi2_gpu - dchi2_cpu| <= 1e-13 * l1
       (l1 = cancellation-aware L1 mass of the sum, computed by the oracle)
   L2  identical accept / reject sequences, except flagged near-ties
   L3  final spectra and chi^2 agree to 1e-9 where the sequences are identical.
@@ -43,7 +43,7 @@ def compare_traces(tg, to, T_sched, amp, stop_on_flagged=True):
     """tg: GPU trace [nw][ns][n_omega], to: oracle trace, same shape.  Returns number of flagged near-ties.
     amp = A / N_omega, the typical coefficient: a bin that once held O(amp) carries an absolute rounding
     history of O(eps * amp) however small it is now (readings T1 and T2, with the bounds and
-    the observed maxima: 8.9e-14 of the tolerance's scale, against 1e-12 here)."""
+    the observed maxima: 8.9e-14 of the tolerance's scale of the candidate values, against 1e-12 there; dchi2: 1e-13 l1)."""
     assert tg.shape == to.shape
     assert (tg["p"] == to["p"]).all() and (tg["s"] == to["s"]).all()
     assert (tg["move"] == to["move"]).all()
@@ -71,7 +71,7 @@ def compare_traces(tg, to, T_sched, amp, stop_on_flagged=True):
         ev = (g["flags"][sl] & 4) != 0
         assert (ev | ((g["flags"][sl] & 1) == 0)).all()            # every feasible move was evaluated
         err = np.abs(g["dchi2"][sl] - o["dchi2"][sl])[ev]
-        tol = 1e-12 * o["l1"][sl][ev]
+        tol = 1e-13 * o["l1"][sl][ev]     # worst case of the arithmetic 2.5e-15 l1; 40x margin (was 1e-12 until round 2)
         assert (err <= tol).all(), f"walker {w}: dchi2 off by up to {np.max(err / o['l1'][sl][ev]):.3e} of l1"
         for fld, dl in (("ap_new", "delta_p"), ("as_new", "delta_s")):
             scale = np.abs(o[dl][sl]) + np.abs(o[fld][sl])
@@ -112,8 +112,8 @@ def test_tiny_full_anneal_trace_and_sequence_parity():
         if flagged == 0:
             assert ((fg & 3) == fo).all()
             assert ((tg["flags"] & 3) == (fg & 3)).all()
-    assert flagged <= 1                                        # expected ~0 (P ~ 1e-2 per whole run)
-    if flagged == 0:
+    assert flagged == 0        # seeded inputs: deterministic; a near-tie within 1e-9 has P ~ 1e-2 per whole run and none occurs
+    if True:
         a, c2 = s.get()
         np.testing.assert_allclose(a, o.a, rtol=0, atol=1e-9 * o.a.max())
         # chi^2 is the running sum chi2_0 + sum dchi2 on both sides (O5 step 8): it carries an absolute rounding
